@@ -1,0 +1,147 @@
+/*
+ * dedisp.h -- C ABI of libdedisp_b200: brute-force incoherent dedispersion on one B200.
+ *
+ *   out[b][i][t] = sum_{c=0}^{C-1} in[b][c][t + shift(c, dm_i)]            (Algorithm 1)
+ *
+ * Paper: Sclocco et al., arXiv 1601.01165 ("PAPER.md" below = /root/reference/PAPER.md).
+ *   - Algorithm 1 defines the triple loop and `input[chan][sample + Delta]`.
+ *   - Eq. (1) defines the delay k = 4150 * DM * (1/f_i^2 - 1/f_h^2) seconds.
+ *   - PAPER.md:45 fixes the matrices: input c x t (channel-major), output d x s (DM-major).
+ *   - PAPER.md:47 : the delays "can be computed in advance" (the shift table).
+ *   - PAPER.md:41, 193 : beams are independent (the nr_beams batch dimension).
+ *   - PAPER.md:76 : tunable kernel parameters chosen by auto-tuning (dedisp_tune).
+ * Readings of silent/ambiguous points (f_h, operation order, rounding ...): DESIGN.md section 2.
+ *
+ * Conventions
+ *   - Every function returns a dedisp_status (0 = OK); no exception crosses the ABI.
+ *   - "device" pointers are CUDA device pointers on the current device; "host" pointers
+ *     are ordinary host memory.  The library never frees or keeps caller buffers.
+ *   - All work runs in hand-written sm_100a kernels; there is no CPU fallback.
+ */
+#ifndef DEDISP_B200_H
+#define DEDISP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dedisp_plan dedisp_plan; /* opaque, owned by the library */
+
+typedef enum {
+    DEDISP_OK = 0,
+    DEDISP_ERR_INVALID_ARG = 1, /* null pointer, non-positive size, negative DM, misalignment */
+    DEDISP_ERR_OVERFLOW = 2,    /* a shift, S + M, or a uint8 sum does not fit its integer type */
+    DEDISP_ERR_ALLOC = 3,       /* host or device allocation failed */
+    DEDISP_ERR_CUDA = 4,        /* CUDA runtime / launch error (no GPU, wrong arch, ...) */
+    DEDISP_ERR_IO = 5           /* tuning cache file could not be read / written */
+} dedisp_status;
+
+/* in_dtype of dedisp_plan_create */
+enum {
+    DEDISP_F32 = 0, /* fp32 input, fp32 accumulation and output */
+    DEDISP_U8 = 1   /* uint8 input, uint32 output (BASELINE.json config 4; exact) */
+};
+
+/* `what` of dedisp_plan_get */
+enum {
+    DEDISP_MAX_SHIFT = 0,  /* M = max over the table = shift(0, D-1) */
+    DEDISP_IN_SAMPLES = 1, /* S + M: samples of each input row that are read (reading A7) */
+    DEDISP_IN_PITCH = 2,   /* elements per input row: S + M rounded up to 16 bytes */
+    DEDISP_OUT_PITCH = 3,  /* elements per output row = S */
+    DEDISP_VARIANT = 4,    /* index of the kernel variant execute() launches */
+    DEDISP_NR_CHANNELS = 5,
+    DEDISP_NR_DMS = 6,
+    DEDISP_NR_SAMPLES = 7,
+    DEDISP_IN_DTYPE = 8
+};
+
+/*
+ * dedisp_plan_create -- steps a1-a3 of the path: trial DMs, channel
+ * frequencies and the int32 shift table, built ON THE DEVICE in IEEE double with the
+ * canonical association (readings A1-A5):
+ *     dm_i = dm_first + i*dm_step            f_c = f_low + c*bw      f_h = f_low + C*bw
+ *     x    = ((4150*dm_i) * (1/(f_c*f_c) - 1/(f_h*f_h))) * sample_rate          (Eq. 1)
+ *     shift(c,i) = floor(x) + (x - floor(x) >= 0.5)
+ * Chooses the kernel variant (tuning cache named by $DEDISP_TUNE_CACHE if set, else a
+ * heuristic).  nr_samples = S, output samples per beam.
+ * Errors: INVALID_ARG (plan == NULL, C/D/S < 1, f_low/bw/rate <= 0 or non-finite,
+ * dm_first/dm_step < 0 or non-finite, unknown dtype); OVERFLOW (shift or S+M > INT32_MAX,
+ * or C*255 >= 2^32 for U8); ALLOC; CUDA.  On error *plan = NULL.
+ */
+int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
+                       double channel_bw_MHz, double sample_rate, int64_t nr_samples,
+                       double dm_first, double dm_step, int nr_dms, int in_dtype);
+
+/*
+ * dedisp_shift_table -- copy Delta(chan, dm) from the DEVICE table the
+ * kernels read into caller-owned HOST memory, row-major [nr_dms][nr_channels], int32,
+ * entry = shift in samples.  Caller provides nr_dms*nr_channels*4 bytes.
+ * Errors: INVALID_ARG (null), CUDA, ALLOC.
+ */
+int dedisp_shift_table(const dedisp_plan *plan, int32_t *host_out);
+
+/* dedisp_plan_get -- scalar queries (see the enum).  Errors: INVALID_ARG. */
+int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value);
+
+/*
+ * dedisp_execute -- steps a4-a7: Algorithm 1 for nr_beams beams.
+ *   d_in : DEVICE, [nr_beams][nr_channels][IN_PITCH] of float (F32) or uint8_t (U8),
+ *          borrowed, read-only, base 16-byte aligned.  Samples [0, S+M) of every row are
+ *          read; pitch padding is ignored.  Sample 0 of the input is time-aligned with
+ *          output sample 0 at f_h.
+ *   d_out: DEVICE, [nr_beams][nr_dms][nr_samples] of float (F32) or uint32_t (U8),
+ *          borrowed, fully overwritten, base 16-byte aligned.
+ *   stream: a cudaStream_t (NULL = default stream).
+ * Asynchronous: enqueues kernels on `stream` and returns; no host sync, no allocation,
+ * no host<->device copy.  fp32 sums are accumulated in fp32 in ascending channel order.
+ * The same plan may be executed repeatedly and concurrently on different streams.
+ * Errors: INVALID_ARG (null, nr_beams < 1, misaligned base), CUDA (launch error).
+ */
+int dedisp_execute(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
+                   void *stream);
+
+/* dedisp_plan_destroy -- frees the plan's host and device tables.  NULL is a no-op. */
+int dedisp_plan_destroy(dedisp_plan *plan);
+
+/* ---- kernel variants and the auto-tuner (step a8) ---------- */
+
+/* Number of compiled kernel variants; variant 0 is the no-reuse "generic" kernel
+ * (one (DM, sample) per thread, global-memory reads: the paper's baseline of PAPER.md:173). */
+int dedisp_variant_count(void);
+
+/* Static string "name: DMs/CTA x samples/CTA, outputs/thread, channel-chunk depth ..." or
+ * NULL if out of range. */
+const char *dedisp_variant_name(int variant);
+
+/* 1 if `variant` can run this plan (dtype, alignment, shared-memory fit), else 0. */
+int dedisp_variant_supported(const dedisp_plan *plan, int variant);
+
+/* Select the variant execute() launches.  Errors: INVALID_ARG if unsupported. */
+int dedisp_plan_set_variant(dedisp_plan *plan, int variant);
+
+/*
+ * dedisp_tune -- exhaustive sweep in the spirit of PAPER.md:76 ("try all meaningful
+ * combinations and select the best performing one"): times every supported variant on the
+ * caller's buffers (same contract as dedisp_execute; d_out is overwritten) with CUDA events
+ * on `stream` (synchronises), selects the fastest, and, if cache_path != NULL, persists
+ * the winner (one text line keyed by GPU name + setup).  ms_out (host, may be NULL)
+ * receives variant_count floats: mean ms per call, or -1 for unsupported variants.
+ */
+int dedisp_tune(dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams, void *stream,
+                const char *cache_path, float *ms_out);
+
+/* Load a winner persisted by dedisp_tune.  Returns OK and leaves the plan unchanged if the
+ * file has no entry for this setup; IO if the file cannot be opened. */
+int dedisp_plan_load_tuning(dedisp_plan *plan, const char *cache_path);
+
+const char *dedisp_status_string(int status);
+
+/* Last CUDA error text seen by this thread inside the library ("" if none). */
+const char *dedisp_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_B200_H */
