@@ -54,7 +54,8 @@ enum {
     DEDISP_NR_CHANNELS = 5,
     DEDISP_NR_DMS = 6,
     DEDISP_NR_SAMPLES = 7,
-    DEDISP_IN_DTYPE = 8
+    DEDISP_IN_DTYPE = 8,
+    DEDISP_MAX_STEP = 9    /* max over (c, i) of shift(c, i+1) - shift(c, i) */
 };
 
 /*
@@ -102,13 +103,34 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value);
 int dedisp_execute(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
                    void *stream);
 
+/*
+ * dedisp_execute_variant -- dedisp_execute with an explicit kernel variant (same contract; used by
+ * the tuner and the parity tests to drive every compiled variant).  INVALID_ARG if the variant
+ * does not support the plan.
+ */
+int dedisp_execute_variant(const dedisp_plan *plan, int variant, const void *d_in, void *d_out,
+                           int nr_beams, void *stream);
+
+/*
+ * dedisp_execute_host -- the same computation for HOST buffers (end-to-end path; the paper keeps
+ * data resident on the device, so this is a convenience, not the hot path):
+ *   h_in : HOST, [nr_beams][nr_channels][IN_PITCH], borrowed (pinned memory copies fastest);
+ *   h_out: HOST, [nr_beams][nr_dms][nr_samples], fully overwritten.
+ * Copies h_in to a plan-owned device workspace (allocated or grown on demand, freed by
+ * dedisp_plan_destroy), runs dedisp_execute on `stream`, copies the result back and SYNCHRONISES
+ * the stream before returning.  Not re-entrant on one plan (the workspace is shared).
+ * Errors: INVALID_ARG, ALLOC (workspace), CUDA.
+ */
+int dedisp_execute_host(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams,
+                        void *stream);
+
 /* dedisp_plan_destroy -- frees the plan's host and device tables.  NULL is a no-op. */
 int dedisp_plan_destroy(dedisp_plan *plan);
 
 /* ---- kernel variants and the auto-tuner (step a8) ---------- */
 
-/* Number of compiled kernel variants; variant 0 is the no-reuse "generic" kernel
- * (one (DM, sample) per thread, global-memory reads: the paper's baseline of PAPER.md:173). */
+/* Number of compiled kernel variants; variants 0 (fp32) and 1 (uint8) are the no-reuse "generic"
+ * kernel (one (DM, sample) per thread, global-memory reads: the paper's baseline of PAPER.md:173). */
 int dedisp_variant_count(void);
 
 /* Static string "name: DMs/CTA x samples/CTA, outputs/thread, channel-chunk depth ..." or
@@ -126,7 +148,8 @@ int dedisp_plan_set_variant(dedisp_plan *plan, int variant);
  * combinations and select the best performing one"): times every supported variant on the
  * caller's buffers (same contract as dedisp_execute; d_out is overwritten) with CUDA events
  * on `stream` (synchronises), selects the fastest, and, if cache_path != NULL, persists
- * the winner (one text line keyed by GPU name + setup).  ms_out (host, may be NULL)
+ * the winner (one text line "key<TAB>variant name<TAB>note" keyed by GPU name + setup, appended;
+ * the last matching line wins on load).  ms_out (host, may be NULL)
  * receives variant_count floats: mean ms per call, or -1 for unsupported variants.
  */
 int dedisp_tune(dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams, void *stream,

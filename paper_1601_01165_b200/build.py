@@ -1,0 +1,70 @@
+"""Builds libdedisp_b200.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the
+repo snapshot).  `python -m paper_1601_01165_b200.build [--force]`."""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(CSRC, "build")
+LIB = os.path.join(HERE, "libdedisp_b200.so")
+
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default"]
+
+# (source, object name, extra defines)
+UNITS = [
+    ("shift_table.cu", "shift_table.o", []),
+    ("plan.cu", "plan.o", []),
+    ("tuner.cu", "tuner.o", []),
+    ("variants_generic.cu", "variants_generic.o", []),
+    ("variants_lds.cu", "variants_lds.o", []),
+    ("variants_u8.cu", "variants_u8.o", []),
+    ("variants_regwin.cu", "variants_regwin0.o", ["-DREGWIN_PART=0"]),
+    ("variants_regwin.cu", "variants_regwin1.o", ["-DREGWIN_PART=1"]),
+    ("variants_regwin.cu", "variants_regwin2.o", ["-DREGWIN_PART=2"]),
+    ("variants_regwin.cu", "variants_regwin3.o", ["-DREGWIN_PART=3"]),
+]
+
+
+def _sources_mtime() -> float:
+    m = os.path.getmtime(os.path.join(HERE, "..", "include", "dedisp.h"))
+    for f in os.listdir(CSRC):
+        if f.endswith((".cu", ".cuh", ".h")):
+            m = max(m, os.path.getmtime(os.path.join(CSRC, f)))
+    return max(m, os.path.getmtime(os.path.abspath(__file__)))
+
+
+def _compile(unit):
+    src, obj, defs = unit
+    cmd = [NVCC, *FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", os.path.join(OBJ, obj)]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    return obj
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _sources_mtime():
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        for obj in ex.map(_compile, UNITS):
+            if verbose:
+                print("compiled", obj)
+    tmp = LIB + ".tmp.%d" % os.getpid()
+    cmd = [NVCC, "-shared", "-o", tmp, *[os.path.join(OBJ, u[1]) for u in UNITS],
+           "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("link failed: %s\n%s" % (" ".join(cmd), r.stderr))
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,95 @@
+// dedisp_internal.h -- plan object, kernel-argument block and the variant registry shared by the
+// translation units of libdedisp_b200.so.  Not part of the public ABI (include/dedisp.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/dedisp.h"
+
+namespace dedisp {
+
+// Kernel families.
+enum Kind {
+    KIND_GENERIC = 0,  // one (DM, sample) per thread, global-memory reads (PAPER.md:173 baseline)
+    KIND_LDS = 1,      // CTA tile staged in shared memory, one shared-memory word per add
+    KIND_REGWIN = 2    // staged tile + per-thread register window reused across the thread's DMs
+};
+
+// Arguments every kernel receives by value.
+struct KArgs {
+    const void *in;          // [B][C][in_pitch]
+    void *out;               // [B][D][S]
+    const int32_t *shift;    // [D][C]          user-visible table
+    const int32_t *shiftT;   // [C][dpitch]     transposed copy, DM axis padded with the last DM
+    int C, D;
+    int S;                   // output samples per beam
+    int in_pitch;            // elements per input row (multiple of 16 bytes)
+    int dpitch;              // ints per shiftT row (multiple of 128, >= D + 128)
+    int lrow;                // shared-memory row pitch in elements (tiled kernels)
+};
+
+// Per-variant numbers derived from the plan's shift table at plan creation.
+struct VariantFit {
+    bool ok = false;     // can run this plan
+    int lrow = 0;        // shared-memory row pitch (elements)
+    size_t smem = 0;     // dynamic shared memory bytes
+};
+
+struct PlanShape {
+    int C, D, S, in_pitch, dtype;
+    int64_t M;               // max shift
+    int max_step;            // max over (c,i) of shift(c,i+1)-shift(c,i)
+    const int32_t *h_shift;  // host copy [D][C]
+};
+
+struct Variant {
+    const char *name;
+    int dtype;        // DEDISP_F32 / DEDISP_U8
+    int kind;
+    int dms_cta;      // DMs per CTA
+    int samples_cta;  // output samples per CTA
+    int dt, tt;       // outputs per thread: dt DMs x tt samples
+    int cc;           // channel-chunk depth (channels per pipeline stage)
+    int stages;
+    int rstep;        // REGWIN: largest per-DM-step shift increment the switch covers
+    int threads;
+    // Fills lrow/smem, returns whether the variant supports the plan.
+    VariantFit (*fit)(const Variant &, const PlanShape &, int span_cta);
+    cudaError_t (*launch)(const KArgs &, int nr_beams, size_t smem, cudaStream_t);
+    cudaError_t (*prepare)(size_t smem);  // cudaFuncSetAttribute for large dynamic smem
+};
+
+const std::vector<Variant> &variants();
+// Each variants_*.cu appends its instantiations.
+void register_generic(std::vector<Variant> &);
+void register_lds(std::vector<Variant> &);
+void register_regwin(std::vector<Variant> &);
+void register_u8(std::vector<Variant> &);
+
+// shift_table.cu
+cudaError_t build_shift_tables(int C, double f_low, double bw, double rate, double dm_first,
+                               double dm_step, int D, int dpitch, int32_t *d_shift,
+                               int32_t *d_shiftT, int *d_flag, cudaStream_t st);
+
+void set_last_error(const char *what, cudaError_t e);
+
+}  // namespace dedisp
+
+struct dedisp_plan {
+    int C, D, dtype;
+    int64_t S, M;
+    int in_pitch, dpitch;
+    double f_low, bw, rate, dm_first, dm_step;
+    int32_t *d_shift = nullptr;
+    int32_t *d_shiftT = nullptr;
+    std::vector<int32_t> h_shift;  // [D][C]
+    int max_step = 0;
+    std::vector<dedisp::VariantFit> fit;  // per variant
+    int variant = 0;
+    // host-buffer path workspace (dedisp_execute_host)
+    void *ws_in = nullptr, *ws_out = nullptr;
+    size_t ws_in_bytes = 0, ws_out_bytes = 0;
+};

@@ -1,0 +1,42 @@
+"""Shipped tuning results (step a8): winners of dedisp_tune on a B200, one text line per
+(GPU, setup), in the format dedisp_tune appends.  `python -m paper_1601_01165_b200.tuning`
+re-tunes the five BASELINE.json configs on the current GPU and rewrites the file."""
+from __future__ import annotations
+
+import os
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SHIPPED = os.path.join(HERE, "tuned", "b200.tsv")
+
+
+def apply_shipped(plan) -> None:
+    """Select the persisted winner for this plan's setup, if the shipped file has one."""
+    if os.path.exists(SHIPPED):
+        plan.load_tuning(SHIPPED)
+
+
+def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 4) -> None:
+    import torch
+
+    from . import dedisp, workloads as wl
+    names = names or list(wl.CONFIGS)
+    tmp = out_path + ".new"
+    if os.path.exists(tmp):
+        os.remove(tmp)
+    for name in names:
+        s = wl.CONFIGS[name]
+        plan = dedisp.Plan(*s.plan_args())
+        nb = min(s.nr_beams, beams_cap)
+        in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
+        d_in = torch.zeros((nb, s.nr_channels, plan.in_pitch), dtype=in_dt, device="cuda")
+        d_out = torch.empty((nb, s.nr_dms, s.nr_samples), dtype=torch.float32, device="cuda")
+        ms = plan.tune(d_in, d_out, nr_beams=nb, cache_path=tmp)
+        for v, t in sorted(ms.items(), key=lambda kv: kv[1]):
+            print("%-10s %9.4f ms  %s" % (name, t, dedisp.variant_name(v)))
+        plan.destroy()
+    os.replace(tmp, out_path)
+
+
+if __name__ == "__main__":
+    retune(sys.argv[1:] or None)

@@ -1,0 +1,145 @@
+"""GPU edge cases through the C-ABI: ragged / degenerate shapes, alignment, errors, tuner."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1601_01165_b200 import workloads as wl
+from test_gpu_parity import TOL, check_full, dd, make_case, out_buffer, to_host  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def run_all(dd, setup, exact=None):
+    plan, table, x, d_in = make_case(dd, setup)
+    ref, sabs = oracle.dedisperse(x, table, setup.nr_samples, want_sabs=True)
+    exact = (setup.in_dtype == wl.U8 or setup.values == "int16") if exact is None else exact
+    for v in plan.supported_variants():
+        d_out = out_buffer(setup, fill=-1 if setup.in_dtype == wl.U8 else float("nan"))
+        plan.execute_variant(v, d_in, d_out, nr_beams=setup.nr_beams)
+        try:
+            check_full(setup, to_host(setup, d_out), ref, sabs, exact)
+        except AssertionError as e:
+            raise AssertionError("%s on %s: %s" % (dd.variant_name(v), setup.name, e))
+    plan.destroy()
+
+
+EDGES = [
+    wl.Setup("one_of_each", 1, 1400.0, 1.0, 1000.0, 1, 0.0, 1.0, 1, values="int16", seed=1),
+    wl.Setup("one_channel", 1, 300.0, 5.0, 5000.0, 700, 0.0, 2.0, 9, values="int16", seed=2),
+    wl.Setup("one_dm", 40, 1400.0, 2.0, 10000.0, 1300, 3.0, 0.0, 1, seed=3),
+    wl.Setup("s_not_mult_of_4", 24, 1400.0, 4.0, 20000.0, 1021, 0.0, 0.5, 37, seed=4),
+    wl.Setup("s_odd_u8", 24, 1400.0, 4.0, 20000.0, 1021, 0.0, 0.5, 37, in_dtype=wl.U8, values="u8", seed=5),
+    wl.Setup("zero_dm_step", 64, 1400.0, 1.0, 20000.0, 2000, 5.0, 0.0, 33, seed=6),   # perfect reuse
+    wl.Setup("all_zero_dm", 64, 1400.0, 1.0, 20000.0, 2000, 0.0, 0.0, 16, values="int16", seed=7),
+    wl.Setup("few_samples", 48, 1400.0, 1.0, 20000.0, 5, 0.0, 0.25, 130, seed=8),
+    wl.Setup("max_u8", 1536, 1220.0, 300.0 / 1536, 24414.0, 64, 0.0, 0.2, 8, in_dtype=wl.U8, values="u8", seed=9),
+    wl.Setup("beams3", 20, 1400.0, 3.0, 20000.0, 900, 0.0, 0.25, 50, nr_beams=3, seed=10),
+    wl.Setup("beams3_u8", 20, 1400.0, 3.0, 20000.0, 900, 0.0, 0.25, 50, nr_beams=3, in_dtype=wl.U8, values="u8", seed=11),
+    wl.Setup("big_steps", 16, 140.0, 0.2, 100000.0, 3000, 0.0, 0.05, 40, seed=12),    # LOFAR-like long shifts
+    wl.Setup("dm_first_nonzero", 32, 1420.0, 1.0, 20000.0, 1500, 100.0, 0.25, 45, seed=13),
+]
+
+
+@pytest.mark.parametrize("setup", EDGES, ids=[s.name for s in EDGES])
+def test_edge_shapes_every_variant(dd, setup):
+    run_all(dd, setup)
+
+
+def test_max_u8_value_saturation_is_exact(dd):
+    """All-255 input over 1536 channels: every output is 1536*255 = 391680 (fits uint32)."""
+    import torch
+    s = wl.Setup("all255", 1536, 1220.0, 300.0 / 1536, 24414.0, 300, 0.0, 0.2, 20, in_dtype=wl.U8)
+    with dd.Plan(*s.plan_args()) as plan:
+        d_in = torch.full((1, s.nr_channels, plan.in_pitch), 255, dtype=torch.uint8, device="cuda")
+        for v in plan.supported_variants():
+            d_out = out_buffer(s, fill=-1)
+            plan.execute_variant(v, d_in, d_out)
+            assert (d_out == 1536 * 255).all(), dd.variant_name(v)
+
+
+def test_execute_is_repeatable_and_stream_ordered(dd):
+    import torch
+    s = wl.scaled(wl.APERTIF, name="rep", nr_channels=64, channel_bw_MHz=300.0 / 64, nr_dms=64,
+                  nr_samples=2000)
+    plan, table, x, d_in = make_case(dd, s)
+    a, b = out_buffer(s, fill=float("nan")), out_buffer(s, fill=float("nan"))
+    st = torch.cuda.Stream()
+    plan.execute(d_in, a)
+    with torch.cuda.stream(st):
+        plan.execute(d_in, b, stream=st)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    plan.destroy()
+
+
+def test_execute_host_matches_device_path(dd):
+    import torch
+    s = wl.scaled(wl.APERTIF, name="host", nr_channels=64, channel_bw_MHz=300.0 / 64, nr_dms=64,
+                  nr_samples=2000, nr_beams=2)
+    plan, table, x, d_in = make_case(dd, s)
+    d_out = out_buffer(s, fill=float("nan"))
+    plan.execute(d_in, d_out, nr_beams=2)
+    h_out = np.full((2, s.nr_dms, s.nr_samples), np.nan, dtype=np.float32)
+    plan.execute_host(x, h_out, nr_beams=2)
+    assert np.array_equal(h_out, d_out.cpu().numpy())
+    plan.destroy()
+
+
+def test_argument_errors_on_device(dd):
+    import torch
+    s = wl.TINY
+    plan, table, x, d_in = make_case(dd, s)
+    d_out = out_buffer(s)
+    lib = dd.load_library()
+    with pytest.raises(dd.DedispError) as e:
+        plan.execute(d_in.data_ptr() + 4, d_out)   # misaligned base
+    assert e.value.status == 1
+    with pytest.raises(dd.DedispError):
+        plan.execute(d_in, d_out, nr_beams=0)
+    with pytest.raises(dd.DedispError):
+        plan.execute(0, d_out)
+    u8 = [v for v in range(dd.variant_count()) if dd.variant_name(v).startswith(("lds_u8", "generic_u8"))]
+    assert u8 and not any(plan.variant_supported(v) for v in u8)
+    with pytest.raises(dd.DedispError):
+        plan.set_variant(u8[0])
+    with pytest.raises(dd.DedispError):
+        plan.execute_variant(u8[0], d_in, d_out)
+    assert lib.dedisp_shift_table(plan._h, None) == 1
+    # an oversized shift must be reported as OVERFLOW, not wrap
+    with pytest.raises(dd.DedispError) as e:
+        dd.Plan(4, 10.0, 0.1, 1e9, 16, 0.0, 1000.0, 64, wl.F32)
+    assert e.value.status == 2
+    plan.destroy()
+
+
+def test_tuner_selects_persists_and_reloads(dd, tmp_path):
+    s = wl.scaled(wl.APERTIF, name="tune", nr_channels=128, channel_bw_MHz=300.0 / 128,
+                  nr_dms=256, nr_samples=4000)
+    plan, table, x, d_in = make_case(dd, s)
+    d_out = out_buffer(s)
+    cache = str(tmp_path / "tune.tsv")
+    ms = plan.tune(d_in, d_out, cache_path=cache)
+    assert set(ms) == set(plan.supported_variants())
+    best = min(ms, key=ms.get)
+    assert plan.variant == best
+    assert os.path.getsize(cache) > 0
+    # the tuned plan still computes the right thing
+    ref, sabs = oracle.dedisperse(x, table, s.nr_samples, want_sabs=True)
+    d_out.fill_(float("nan"))
+    plan.execute(d_in, d_out)
+    check_full(s, to_host(s, d_out), ref, sabs, False)
+    # a fresh plan picks the winner up from the cache; another setup is left alone
+    with dd.Plan(*s.plan_args()) as p2:
+        p2.set_variant(0)
+        p2.load_tuning(cache)
+        assert p2.variant == best
+    with dd.Plan(*wl.TINY.plan_args()) as p3:
+        before = p3.variant
+        p3.load_tuning(cache)
+        assert p3.variant == before
+    with pytest.raises(dd.DedispError) as e:
+        plan.load_tuning(str(tmp_path / "missing.tsv"))
+    assert e.value.status == 5
+    plan.destroy()

@@ -1,0 +1,226 @@
+"""GPU parity tests: the CUDA path, called through the C-ABI, against the CPU oracle on the same
+seeded inputs.  Acceptance (BASELINE.json north_star): shift tables bit-exact; integer-valued and
+uint8 inputs bit-exact; Gaussian fp32 within 1e-5 * sum_c |x_c| per output."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1601_01165_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5  # x sum_c |x_c| per output (BASELINE.json; reading A18)
+
+
+@pytest.fixture(scope="module")
+def dd():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1601_01165_b200 import build, dedisp
+    build.build()
+    dedisp.load_library()
+    return dedisp
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def make_case(dd, setup):
+    """plan, oracle table, host input, device input."""
+    torch = _torch()
+    plan = dd.Plan(*setup.plan_args())
+    table = oracle.shift_table(*setup.table_args())
+    pulse = table[setup.pulse[0]] if setup.pulse is not None else None
+    assert plan.in_samples == setup.nr_samples + int(table.max())
+    x = wl.make_input(setup, plan.in_samples, plan.in_pitch, pulse_shifts=pulse)
+    d_in = torch.from_numpy(x).cuda()
+    return plan, table, x, d_in
+
+
+def out_buffer(setup, fill=None):
+    torch = _torch()
+    dt = torch.float32 if setup.in_dtype == wl.F32 else torch.int32  # uint32 bits in an int32 tensor
+    shape = (setup.nr_beams, setup.nr_dms, setup.nr_samples)
+    if fill is None:
+        return torch.empty(shape, dtype=dt, device="cuda")
+    return torch.full(shape, fill, dtype=dt, device="cuda")
+
+
+def to_host(setup, d_out):
+    a = d_out.cpu().numpy()
+    return a.view(np.uint32) if setup.in_dtype == wl.U8 else a
+
+
+def check_full(setup, got, ref, sabs, exact):
+    if exact:
+        if setup.in_dtype == wl.U8:
+            assert np.array_equal(got.astype(np.uint64), ref)
+        else:
+            assert np.array_equal(got.astype(np.float64), ref)
+    else:
+        err = np.abs(got.astype(np.float64) - ref)
+        bad = err > TOL * sabs
+        assert not bad.any(), "max err/sabs = %g" % float((err / np.maximum(sabs, 1e-30)).max())
+
+
+# ------------------------------------------------------------------ shift tables
+@pytest.mark.parametrize("name", ["tiny", "apertif", "lofar", "survey8", "batch40"])
+def test_shift_table_bit_exact(dd, name):
+    s = wl.CONFIGS[name]
+    with dd.Plan(*s.plan_args()) as plan:
+        got = plan.shift_table()
+        ref = oracle.shift_table(*s.table_args())
+        assert got.dtype == np.int32 and got.shape == ref.shape
+        assert np.array_equal(got, ref)
+        assert plan.max_shift == int(ref.max())
+        assert plan.in_samples == s.nr_samples + int(ref.max())
+        al = 16 if s.in_dtype == wl.U8 else 4
+        assert plan.in_pitch % al == 0 and 0 <= plan.in_pitch - plan.in_samples < al
+        assert plan.max_step == int(np.diff(ref, axis=0).max())
+
+
+def test_shift_table_odd_setups_bit_exact(dd):
+    rng = np.random.default_rng(7)
+    for _ in range(12):
+        C = int(rng.integers(1, 70))
+        D = int(rng.integers(1, 300))
+        args = (C, float(rng.uniform(100, 2000)), float(rng.uniform(0.01, 3.0)),
+                float(rng.uniform(500, 300000)), float(rng.uniform(0, 5)), float(rng.uniform(0, 0.7)), D)
+        with dd.Plan(args[0], args[1], args[2], args[3], 64, args[4], args[5], D, wl.F32) as plan:
+            assert np.array_equal(plan.shift_table(), oracle.shift_table(*args))
+
+
+# ------------------------------------------------------------------ config 1: tiny, bit-exact
+def test_tiny_every_variant_bit_exact_and_pulse(dd):
+    s = wl.TINY
+    plan, table, x, d_in = make_case(dd, s)
+    ref = oracle.dedisperse(x, table, s.nr_samples)
+    ran = []
+    for v in plan.supported_variants():
+        d_out = out_buffer(s, fill=-1.0)
+        plan.execute_variant(v, d_in, d_out)
+        got = to_host(s, d_out)
+        assert np.array_equal(got.astype(np.float64), ref), dd.variant_name(v)
+        ran.append(dd.variant_name(v))
+    assert any(n.startswith("regwin") for n in ran) and any(n.startswith("lds") for n in ran)
+    # the default (heuristic or tuned) launch, and the injected pulse (readings A13/A14)
+    d_out = out_buffer(s, fill=-1.0)
+    plan.execute(d_in, d_out)
+    got = to_host(s, d_out)[0]
+    assert np.array_equal(got.astype(np.float64), ref[0])
+    dm_i, t_arr, amp = s.pulse
+    assert np.unravel_index(np.argmax(got), got.shape) == (dm_i, t_arr)
+    assert (got == got.max()).sum() == 1
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ scaled configs, every variant
+SCALED = [
+    # several DM tiles and sample tiles with ragged tails in both, channels not a chunk multiple
+    wl.scaled(wl.APERTIF, name="apertif_s", nr_channels=100, channel_bw_MHz=300.0 / 100,
+              nr_dms=203, nr_samples=3001),
+    wl.scaled(wl.APERTIF, name="apertif_s4", nr_channels=61, channel_bw_MHz=300.0 / 61,
+              nr_dms=77, nr_samples=2600),
+    wl.scaled(wl.LOFAR, name="lofar_s", nr_channels=32, nr_dms=70, nr_samples=5003),
+    wl.scaled(wl.SURVEY8, name="survey8_s", nr_channels=150, channel_bw_MHz=300.0 / 150,
+              nr_dms=130, nr_samples=3007),
+    wl.scaled(wl.SURVEY8, name="survey8_s16", nr_channels=33, channel_bw_MHz=300.0 / 33,
+              nr_dms=40, nr_samples=4096),
+]
+
+
+@pytest.mark.parametrize("setup", SCALED, ids=[s.name for s in SCALED])
+def test_scaled_every_variant(dd, setup):
+    plan, table, x, d_in = make_case(dd, setup)
+    ref, sabs = oracle.dedisperse(x, table, setup.nr_samples, want_sabs=True)
+    exact = setup.in_dtype == wl.U8
+    vs = plan.supported_variants()
+    assert len(vs) >= 3
+    for v in vs:
+        d_out = out_buffer(setup, fill=-1 if exact else float("nan"))
+        plan.execute_variant(v, d_in, d_out)
+        try:
+            check_full(setup, to_host(setup, d_out), ref, sabs, exact)
+        except AssertionError as e:
+            raise AssertionError("%s: %s" % (dd.variant_name(v), e))
+    plan.destroy()
+
+
+def test_integer_valued_fp32_bit_exact_every_variant(dd):
+    s = wl.scaled(wl.APERTIF, name="apertif_int", nr_channels=128, channel_bw_MHz=300.0 / 128,
+                  nr_dms=96, nr_samples=2500, values="int16")
+    plan, table, x, d_in = make_case(dd, s)
+    ref = oracle.dedisperse(x, table, s.nr_samples)
+    for v in plan.supported_variants():
+        d_out = out_buffer(s, fill=-1.0)
+        plan.execute_variant(v, d_in, d_out)
+        assert np.array_equal(to_host(s, d_out).astype(np.float64), ref), dd.variant_name(v)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ full-size configs, sampled
+@pytest.mark.parametrize("name", ["apertif", "lofar", "survey8"])
+def test_full_size_sampled_points(dd, name):
+    """BASELINE.json sizes in the launch configuration bench.py times (plan default after
+    load_tuning of the shipped cache), compared on sampled outputs the oracle computes one by one,
+    plus whole rows (DM 0 = plain channel sum, and the last DM)."""
+    torch = _torch()
+    from paper_1601_01165_b200 import tuning
+    s = wl.CONFIGS[name]
+    plan, table, x, d_in = make_case(dd, s)
+    tuning.apply_shipped(plan)
+    exact = s.in_dtype == wl.U8
+    d_out = out_buffer(s, fill=-1 if exact else float("nan"))
+    plan.execute(d_in, d_out)
+    torch.cuda.synchronize()
+    pts = wl.sample_points(s, 20000)
+    got = to_host(s, d_out)
+    g = got[pts[:, 0], pts[:, 1], pts[:, 2]]
+    ref, sabs = oracle.dedisperse_points(x, table, s.nr_samples, pts, want_sabs=True)
+    if exact:
+        assert np.array_equal(g.astype(np.uint64), ref)
+    else:
+        assert (np.abs(g.astype(np.float64) - ref) <= TOL * sabs).all()
+        assert np.isfinite(got).all()
+    # property that holds at any size: the DM-0 row is the plain channel sum (shifts are all 0)
+    row0 = x[0, :, :s.nr_samples].astype(np.float64 if not exact else np.uint64).sum(axis=0)
+    if exact:
+        assert np.array_equal(got[0, 0].astype(np.uint64), row0)
+    else:
+        assert np.allclose(got[0, 0], row0, rtol=0, atol=1e-3)
+    plan.destroy()
+
+
+def test_batch40_beams_match_single_beam_calls(dd):
+    """Config 5: 40 beams in one dedisp_execute; beam b must be bit-identical to a single-beam call
+    on beam b (independent beams), and sampled points must match the oracle."""
+    torch = _torch()
+    from paper_1601_01165_b200 import tuning
+    s = wl.BATCH40
+    plan = dd.Plan(*s.plan_args())
+    tuning.apply_shipped(plan)
+    table = oracle.shift_table(*s.table_args())
+    d_in = torch.empty((s.nr_beams, s.nr_channels, plan.in_pitch), dtype=torch.float32, device="cuda")
+    keep = {}
+    for b in range(s.nr_beams):
+        xb = wl.make_input(s, plan.in_samples, plan.in_pitch, beams=range(b, b + 1))
+        d_in[b].copy_(torch.from_numpy(xb[0]))
+        if b in (0, 17, 39):
+            keep[b] = xb
+    d_out = out_buffer(s, fill=float("nan"))
+    plan.execute(d_in, d_out, nr_beams=s.nr_beams)
+    torch.cuda.synchronize()
+    single = torch.empty((1, s.nr_dms, s.nr_samples), dtype=torch.float32, device="cuda")
+    for b, xb in keep.items():
+        single.fill_(float("nan"))
+        plan.execute(d_in[b], single, nr_beams=1)
+        assert torch.equal(single[0], d_out[b]), "beam %d differs from its single-beam call" % b
+        one = wl.scaled(s, nr_beams=1)
+        pts = wl.sample_points(one, 4000, seed=b)
+        got = single.cpu().numpy()[pts[:, 0], pts[:, 1], pts[:, 2]]
+        ref, sabs = oracle.dedisperse_points(xb, table, s.nr_samples, pts, want_sabs=True)
+        assert (np.abs(got.astype(np.float64) - ref) <= TOL * sabs).all()
+    assert torch.isfinite(d_out).all()
+    plan.destroy()
