@@ -31,10 +31,24 @@ UNITS = [
 ]
 
 
+def _tree_variants():
+    """(part, WD, WT, DT, TT, CC, NS, QMAX, MINB) rows of TREE_VARIANTS in variants_tree.cu."""
+    import re
+    text = open(os.path.join(CSRC, "variants_tree.cu")).read()
+    rows = re.findall(r"^\s*X\((\d+(?:,\s*\d+){8})\)", text, flags=re.M)
+    return [tuple(int(x) for x in r.split(",")) for r in rows]
+
+
+TREE = _tree_variants()
+UNITS += [("variants_tree.cu", "variants_tree%d.o" % t[0], ["-DTREE_PART=%d" % t[0]]) for t in TREE]
+# (DT, TT, QMAX) of every TreeTile: gen_tree.py writes their add lattices
+TREE_COMBOS = sorted({"%d,%d,%d" % (t[3], t[4], t[7]) for t in TREE})
+
+
 def _sources_mtime() -> float:
     m = os.path.getmtime(os.path.join(HERE, "..", "include", "dedisp.h"))
     for f in os.listdir(CSRC):
-        if f.endswith((".cu", ".cuh", ".h")):
+        if f.endswith((".cu", ".cuh", ".h", ".py")):
             m = max(m, os.path.getmtime(os.path.join(CSRC, f)))
     return max(m, os.path.getmtime(os.path.abspath(__file__)))
 
@@ -52,6 +66,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _sources_mtime():
         return LIB
     os.makedirs(OBJ, exist_ok=True)
+    r = subprocess.run([sys.executable, os.path.join(CSRC, "gen_tree.py"),
+                        os.path.join(OBJ, "tree_gen.cuh"), *TREE_COMBOS],
+                       capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("gen_tree.py failed:\n%s\n%s" % (r.stdout, r.stderr))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         for obj in ex.map(_compile, UNITS):
             if verbose:

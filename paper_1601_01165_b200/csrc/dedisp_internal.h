@@ -15,7 +15,8 @@ namespace dedisp {
 enum Kind {
     KIND_GENERIC = 0,  // one (DM, sample) per thread, global-memory reads (PAPER.md:173 baseline)
     KIND_LDS = 1,      // CTA tile staged in shared memory, one shared-memory word per add
-    KIND_REGWIN = 2    // staged tile + per-thread register window reused across the thread's DMs
+    KIND_REGWIN = 2,   // staged tile + per-thread register window reused across the thread's DMs
+    KIND_TREE = 3      // register window, offsets selected by a generated branch lattice
 };
 
 // Arguments every kernel receives by value.
@@ -29,6 +30,8 @@ struct KArgs {
     int in_pitch;            // elements per input row (multiple of 16 bytes)
     int dpitch;              // ints per shiftT row (multiple of 128, >= D + 128)
     int lrow;                // shared-memory row pitch in elements (tiled kernels)
+    const uint32_t *desc;    // KIND_TREE: [C][descpitch] descriptors for the variant's tile
+    int descpitch;
 };
 
 // Per-variant numbers derived from the plan's shift table at plan creation.
@@ -43,6 +46,26 @@ struct PlanShape {
     int64_t M;               // max shift
     int max_step;            // max over (c,i) of shift(c,i+1)-shift(c,i)
     const int32_t *h_shift;  // host copy [D][C]
+    const struct TreeInfo *tree;  // KIND_TREE tables
+};
+
+// Descriptor table of the KIND_TREE kernels for one (DT, DMs per CTA) pair, built by desc_kernel
+// at plan creation.
+struct TreeTable {
+    int dt = 0, dms_cta = 0;
+    uint32_t *d_desc = nullptr;  // [C][pitch]
+    int pitch = 0;
+    bool valid = false;          // every woff fits 16 bits
+};
+struct TreeInfo {
+    bool valid = false;  // every channel's increments are {q_c, q_c + 1}, q_c <= 15
+    int qmax = -1;       // max_c q_c
+    std::vector<TreeTable> tables;
+    const TreeTable *find(int dt, int dms_cta) const {
+        for (const TreeTable &t : tables)
+            if (t.dt == dt && t.dms_cta == dms_cta) return &t;
+        return nullptr;
+    }
 };
 
 struct Variant {
@@ -68,11 +91,18 @@ void register_generic(std::vector<Variant> &);
 void register_lds(std::vector<Variant> &);
 void register_regwin(std::vector<Variant> &);
 void register_u8(std::vector<Variant> &);
+void register_tree(std::vector<Variant> &);
 
 // shift_table.cu
 cudaError_t build_shift_tables(int C, double f_low, double bw, double rate, double dm_first,
                                double dm_step, int D, int dpitch, int32_t *d_shift,
                                int32_t *d_shiftT, int *d_flag, cudaStream_t st);
+
+cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch, int *d_qc,
+                              int *d_flags, cudaStream_t st);
+cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int D, int dpitch,
+                            int dt, int dms_cta, int descpitch, uint32_t *d_desc, int *d_flags,
+                            cudaStream_t st);
 
 void set_last_error(const char *what, cudaError_t e);
 
@@ -88,6 +118,7 @@ struct dedisp_plan {
     std::vector<int32_t> h_shift;  // [D][C]
     int max_step = 0;
     std::vector<dedisp::VariantFit> fit;  // per variant
+    dedisp::TreeInfo tree;
     int variant = 0;
     // host-buffer path workspace (dedisp_execute_host)
     void *ws_in = nullptr, *ws_out = nullptr;

@@ -23,6 +23,26 @@ void register_regwin0(std::vector<Variant> &);
 void register_regwin1(std::vector<Variant> &);
 void register_regwin2(std::vector<Variant> &);
 void register_regwin3(std::vector<Variant> &);
+#define DEDISP_TREE_PARTS 12  // rows of TREE_VARIANTS in variants_tree.cu
+void register_tree0(std::vector<Variant> &);
+void register_tree1(std::vector<Variant> &);
+void register_tree2(std::vector<Variant> &);
+void register_tree3(std::vector<Variant> &);
+void register_tree4(std::vector<Variant> &);
+void register_tree5(std::vector<Variant> &);
+void register_tree6(std::vector<Variant> &);
+void register_tree7(std::vector<Variant> &);
+void register_tree8(std::vector<Variant> &);
+void register_tree9(std::vector<Variant> &);
+void register_tree10(std::vector<Variant> &);
+void register_tree11(std::vector<Variant> &);
+void register_tree(std::vector<Variant> &r) {
+    void (*parts[DEDISP_TREE_PARTS])(std::vector<Variant> &) = {
+        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4,
+        register_tree5, register_tree6, register_tree7, register_tree8, register_tree9,
+        register_tree10, register_tree11};
+    for (auto f : parts) f(r);
+}
 void register_regwin(std::vector<Variant> &r) {
     register_regwin0(r);
     register_regwin1(r);
@@ -38,6 +58,7 @@ const std::vector<Variant> &variants() {
         register_lds(reg);
         register_u8(reg);
         register_regwin(reg);
+        register_tree(reg);
     });
     return reg;
 }
@@ -58,6 +79,7 @@ static PlanShape shape_of(const dedisp_plan *pl) {
     PlanShape p;
     p.C = pl->C; p.D = pl->D; p.S = (int)pl->S; p.in_pitch = pl->in_pitch; p.dtype = pl->dtype;
     p.M = pl->M; p.max_step = pl->max_step; p.h_shift = pl->h_shift.data();
+    p.tree = &pl->tree;
     return p;
 }
 
@@ -78,6 +100,49 @@ static void compute_fits(dedisp_plan *pl) {
     }
 }
 
+// KIND_TREE tables: per-channel slope classes, then one descriptor table per (DT, DMs per CTA)
+// pair some registered variant uses.
+static cudaError_t build_tree_tables(dedisp_plan *pl) {
+    if (pl->C > 65535) return cudaSuccess;  // grid.y of desc_kernel; such plans use other kinds
+    int *d_flags = nullptr, *d_qc = nullptr;
+    int h[2] = {0, 0};
+    cudaError_t e;
+    if ((e = cudaMalloc(&d_flags, 8)) != cudaSuccess || (e = cudaMalloc(&d_qc, (size_t)pl->C * 4)) != cudaSuccess ||
+        (e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
+        (e = build_chan_slopes(pl->d_shiftT, pl->C, pl->D, pl->dpitch, d_qc, d_flags, 0)) != cudaSuccess ||
+        (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess) {
+        set_last_error("build_chan_slopes", e);
+        cudaFree(d_flags);
+        cudaFree(d_qc);
+        return e;
+    }
+    pl->tree.qmax = h[0];
+    pl->tree.valid = h[1] == 0;
+    if (pl->tree.valid) {
+        for (const Variant &v : variants()) {
+            if (v.kind != KIND_TREE || v.dtype != pl->dtype || v.rstep < pl->tree.qmax) continue;
+            if (pl->tree.find(v.dt, v.dms_cta)) continue;
+            TreeTable t;
+            t.dt = v.dt;
+            t.dms_cta = v.dms_cta;
+            const int nG = (pl->D + v.dt - 1) / v.dt;
+            t.pitch = (nG + 31) / 32 * 32 + 32;
+            if ((e = cudaMalloc(&t.d_desc, (size_t)pl->C * t.pitch * 4)) != cudaSuccess) break;
+            pl->tree.tables.push_back(t);  // owned by the plan from here on
+            if ((e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
+                (e = build_tree_desc(pl->d_shiftT, d_qc, pl->C, pl->D, pl->dpitch, v.dt, v.dms_cta,
+                                     t.pitch, t.d_desc, d_flags, 0)) != cudaSuccess ||
+                (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess)
+                break;
+            pl->tree.tables.back().valid = h[1] == 0;
+        }
+        if (e != cudaSuccess) set_last_error("build_tree_desc", e);
+    }
+    cudaFree(d_flags);
+    cudaFree(d_qc);
+    return e;
+}
+
 // Untuned default: a rough cost model (adds / kind rate, tile padding, wave quantisation).
 static int heuristic_variant(const dedisp_plan *pl) {
     const auto &vs = variants();
@@ -86,7 +151,7 @@ static int heuristic_variant(const dedisp_plan *pl) {
     for (size_t v = 0; v < vs.size(); ++v) {
         if (!pl->fit[v].ok) continue;
         const Variant &x = vs[v];
-        double rate = x.kind == KIND_REGWIN ? 2.5 : x.kind == KIND_LDS ? 1.0 : 0.25;
+        double rate = x.kind == KIND_TREE ? 2.0 : x.kind == KIND_REGWIN ? 0.8 : x.kind == KIND_LDS ? 1.0 : 0.25;
         double nd = std::ceil((double)pl->D / x.dms_cta), nt = std::ceil((double)pl->S / x.samples_cta);
         double work = nd * x.dms_cta * nt * x.samples_cta;  // padded outputs
         double ctas = nd * nt;
@@ -167,6 +232,7 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     in_samples = nr_samples + pl->M;
     if (in_samples + al > INT32_MAX) { status = DEDISP_ERR_OVERFLOW; goto fail; }
     pl->in_pitch = (int)((in_samples + al - 1) / al * al);
+    if (build_tree_tables(pl) != cudaSuccess) goto cuda_fail;
     compute_fits(pl);
     pl->variant = heuristic_variant(pl);
     if (const char *cache = getenv("DEDISP_TUNE_CACHE"))
@@ -217,6 +283,9 @@ static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void
     a.in = d_in; a.out = d_out; a.shift = plan->d_shift; a.shiftT = plan->d_shiftT;
     a.C = plan->C; a.D = plan->D; a.S = (int)plan->S; a.in_pitch = plan->in_pitch;
     a.dpitch = plan->dpitch; a.lrow = f.lrow;
+    const TreeTable *tt = x.kind == KIND_TREE ? plan->tree.find(x.dt, x.dms_cta) : nullptr;
+    a.desc = tt ? tt->d_desc : nullptr;
+    a.descpitch = tt ? tt->pitch : 0;
     // grid.z carries the beams (step a7): at most 65535 per launch
     const size_t in_beam = (size_t)plan->C * plan->in_pitch * (plan->dtype == DEDISP_U8 ? 1 : 4);
     const size_t out_beam = (size_t)plan->D * plan->S * 4;
@@ -298,6 +367,8 @@ int dedisp_plan_destroy(dedisp_plan *plan) {
     if (!plan) return DEDISP_OK;
     if (plan->d_shift) cudaFree(plan->d_shift);
     if (plan->d_shiftT) cudaFree(plan->d_shiftT);
+    for (auto &t : plan->tree.tables)
+        if (t.d_desc) cudaFree(t.d_desc);
     if (plan->ws_in) cudaFree(plan->ws_in);
     if (plan->ws_out) cudaFree(plan->ws_out);
     delete plan;

@@ -52,4 +52,87 @@ cudaError_t build_shift_tables(int C, double f_low, double bw, double rate, doub
     return cudaGetLastError();
 }
 
+// KIND_TREE tables (kernel_tree.cuh).
+// chan_slope_kernel: one block per channel c.  q_c = min over i of shift(c,i+1) - shift(c,i); the
+// tree kernels need every increment of the channel to be q_c or q_c + 1 (true for a rounded linear
+// function of the DM index).  flags[0] = max_c q_c, flags[1] = 1 if some channel violates it.
+__global__ void chan_slope_kernel(const int32_t *shiftT, int D, int dpitch, int *qc, int *flags) {
+    const int c = blockIdx.x;
+    const int32_t *row = shiftT + (size_t)c * dpitch;
+    int mn = 0x7fffffff, mx = 0;
+    for (int i = threadIdx.x; i + 1 < D; i += blockDim.x) {
+        int d = row[i + 1] - row[i];
+        mn = d < mn ? d : mn;
+        mx = d > mx ? d : mx;
+    }
+    __shared__ int smn[128], smx[128];
+    smn[threadIdx.x] = mn;
+    smx[threadIdx.x] = mx;
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            smn[threadIdx.x] = min(smn[threadIdx.x], smn[threadIdx.x + o]);
+            smx[threadIdx.x] = max(smx[threadIdx.x], smx[threadIdx.x + o]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        mn = smn[0];
+        mx = smx[0];
+        if (mn == 0x7fffffff) mn = 0;  // D == 1
+        if (mn < 0 || mn > 15 || mx - mn > 1) {
+            atomicOr(&flags[1], 1);
+            mn = 0;
+        }
+        atomicMax(&flags[0], mn);
+        qc[c] = mn;
+    }
+}
+
+// desc_kernel: one thread per (channel c, DM group G of dt DMs); the group belongs to the CTA tile
+// of dms_cta DMs that starts at DM lo = (G*dt / dms_cta) * dms_cta.
+//   desc[c][G] = woff << 16 | q_c << 12 | bits
+//   woff = shift(c, G*dt) - (shift(c, lo) & ~3): offset of the group's first DM in the staged row,
+//          whose element 0 is input sample T0 + (shift(c, lo) & ~3);
+//   bits: increment j of the group = q_c + bit (j-1).
+// DMs past D (ragged last group, padding groups) continue with increment q_c: their outputs are
+// never stored and their window offsets stay inside the lattice.  flags[1] |= 1 if woff >= 2^16.
+__global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, int dpitch, int dt,
+                            int dms_cta, int descpitch, uint32_t *desc, int *flags) {
+    int G = blockIdx.x * blockDim.x + threadIdx.x;
+    int c = blockIdx.y;
+    if (G >= descpitch) return;
+    const int32_t *row = shiftT + (size_t)c * dpitch;
+    const long d0 = (long)G * dt;
+    const long lo = d0 / dms_cta * dms_cta;
+    const int e0 = row[d0 < D ? d0 : D - 1];
+    const int base = row[lo < D ? lo : D - 1] & ~3;
+    const int q = qc[c];
+    uint32_t bits = 0;
+    for (int j = 1; j < dt && d0 + j < D; ++j) {
+        int b = (row[d0 + j] - row[d0 + j - 1]) - q;
+        b = b < 0 ? 0 : b > 1 ? 1 : b;  // only when flags[1] is already set
+        bits |= (uint32_t)b << (j - 1);
+    }
+    const int woff = e0 - base;
+    if (woff < 0 || woff > 0xffff) atomicOr(&flags[1], 1);
+    desc[(size_t)c * descpitch + G] = ((uint32_t)woff & 0xffffu) << 16 | (uint32_t)q << 12 | bits;
+}
+
+cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch, int *d_qc,
+                              int *d_flags, cudaStream_t st) {
+    chan_slope_kernel<<<C, 128, 0, st>>>(d_shiftT, D, dpitch, d_qc, d_flags);
+    return cudaGetLastError();
+}
+
+cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int D, int dpitch,
+                            int dt, int dms_cta, int descpitch, uint32_t *d_desc, int *d_flags,
+                            cudaStream_t st) {
+    dim3 block(128);
+    dim3 grid((descpitch + 127) / 128, C);
+    desc_kernel<<<grid, block, 0, st>>>(d_shiftT, d_qc, C, D, dpitch, dt, dms_cta, descpitch,
+                                        d_desc, d_flags);
+    return cudaGetLastError();
+}
+
 }  // namespace dedisp
