@@ -32,11 +32,12 @@ UNITS = [
 
 
 def _tree_variants():
-    """(part, WD, WT, DT, TT, CC, NS, QMAX, MINB) rows of TREE_VARIANTS in variants_tree.cu."""
+    """(part, WD, WT, DT, TT, CC, NS, QMAX, MINB) rows of TREE_VARIANTS in variants_tree.cu (the input
+    type column is skipped)."""
     import re
     text = open(os.path.join(CSRC, "variants_tree.cu")).read()
-    rows = re.findall(r"^\s*X\((\d+(?:,\s*\d+){8})\)", text, flags=re.M)
-    return [tuple(int(x) for x in r.split(",")) for r in rows]
+    rows = re.findall(r"^\s*X\((\d+),\s*\w+((?:,\s*\d+){8})\)", text, flags=re.M)
+    return [tuple(int(x) for x in (a + b).split(",")) for a, b in rows]
 
 
 TREE = _tree_variants()

@@ -101,8 +101,8 @@ cudaError_t build_shift_tables(int C, double f_low, double bw, double rate, doub
 cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch, int *d_qc,
                               int *d_flags, cudaStream_t st);
 cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int D, int dpitch,
-                            int dt, int dms_cta, int descpitch, uint32_t *d_desc, int *d_flags,
-                            cudaStream_t st);
+                            int dt, int dms_cta, int al, int descpitch, uint32_t *d_desc,
+                            int *d_flags, cudaStream_t st);
 
 void set_last_error(const char *what, cudaError_t e);
 

@@ -21,10 +21,13 @@
 
 namespace dedisp {
 
-template <int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_, int QMAX_, int MINB_>
+template <typename In_, int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_, int QMAX_,
+          int MINB_>
 struct TreeTile {
-    typedef float In;
-    typedef float Acc;
+    typedef In_ In;                              // float, or uint8_t converted to fp32 at staging
+    typedef typename AccOf<In_>::type Acc;       // output type: float / uint32_t
+    static constexpr bool U8 = sizeof(In_) == 1;
+    static constexpr int AL = 16 / (int)sizeof(In_);  // elements per 16 bytes of input
     static constexpr int WD = WD_, WT = WT_, DT = DT_, TT = TT_, CC = CC_, NSTAGE = NSTAGE_,
                          QMAX = QMAX_, MINB = MINB_;
     static constexpr int NW = WD * WT;
@@ -36,21 +39,31 @@ struct TreeTile {
     static_assert(WD % 4 == 0, "descriptor rows are copied in 16-byte units");
     static_assert(CC <= 32, "one lane per channel of a chunk issues its copies");
     static_assert(DT <= 13, "12 increment bits per descriptor");
+    static_assert(SAMPLES_CTA % AL == 0, "time tiles start on 16-byte boundaries of the input");
 };
 
+// Shared memory (dynamic): mbarriers | NSTAGE stages { CC input rows of lrow elements | CC x WD
+// descriptors } | for uint8 input two fp32 buffers { CC rows of lrow floats | CC x WD descriptors }
+// the compute loop reads (the stage rows are converted into them, chunk k into buffer k & 1).
 template <typename T>
 __host__ __device__ inline size_t tree_stage_bytes(int lrow) {
+    return (size_t)T::CC * ((size_t)lrow * sizeof(typename T::In) + (size_t)T::WD * 4);
+}
+template <typename T>
+__host__ __device__ inline size_t tree_fbuf_bytes(int lrow) {
     return (size_t)T::CC * ((size_t)lrow * 4 + (size_t)T::WD * 4);
 }
 template <typename T>
 __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
-    return T::NSTAGE * tree_stage_bytes<T>(lrow) + 2 * T::NSTAGE * sizeof(uint64_t) + 16;
+    return T::NSTAGE * tree_stage_bytes<T>(lrow) + (T::U8 ? 2 * tree_fbuf_bytes<T>(lrow) : 0) +
+           2 * T::NSTAGE * sizeof(uint64_t) + 16;
 }
 
 // Issue the copies of chunk k into its stage (called by one whole warp; lane l < CC stages channel
 // k*CC + l: its input span and its WD descriptors).
 template <typename T>
-__device__ __forceinline__ void tree_issue(const KArgs &a, const float *in, const uint32_t *desc,
+__device__ __forceinline__ void tree_issue(const KArgs &a, const typename T::In *in,
+                                           const uint32_t *desc,
                                            int descpitch, int k, int lane, int T0, int dm_lo,
                                            int g_lo, unsigned char *stages, size_t sbytes,
                                            size_t data_bytes, uint64_t *full) {
@@ -60,14 +73,15 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const float *in, cons
     if (lane < T::CC && c < a.C) {
         const int32_t *trow = a.shiftT + (size_t)c * a.dpitch + dm_lo;
         const int smin = trow[0], smax = trow[T::DMS_CTA - 1];
-        const int g0 = T0 + (smin & ~3);
+        const int g0 = T0 + (smin & ~(T::AL - 1));
         int end = T0 + T::SAMPLES_CTA + smax;
         end = end < a.in_pitch ? end : a.in_pitch;
-        int len = (end - g0 + 3) & ~3;
+        int len = (end - g0 + T::AL - 1) & ~(T::AL - 1);
         len = len < a.lrow ? len : a.lrow;
         unsigned char *st = stages + (size_t)s * sbytes;
-        const uint32_t nb = (uint32_t)len * 4;
-        bulk_g2s(st + (size_t)lane * a.lrow * 4, in + (size_t)c * a.in_pitch + g0, nb, &full[s]);
+        const uint32_t nb = (uint32_t)len * sizeof(typename T::In);
+        bulk_g2s(st + (size_t)lane * a.lrow * sizeof(typename T::In),
+                 in + (size_t)c * a.in_pitch + g0, nb, &full[s]);
         bulk_g2s(st + data_bytes + (size_t)lane * T::WD * 4, desc + (size_t)c * descpitch + g_lo,
                  T::WD * 4, &full[s]);
         bytes = nb + T::WD * 4;
@@ -87,14 +101,15 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     uint64_t *empty = full + T::NSTAGE;
     unsigned char *stages = smem_raw + ((2 * T::NSTAGE * sizeof(uint64_t) + 15) & ~(size_t)15);
     const size_t sbytes = tree_stage_bytes<T>(a.lrow);
-    const size_t data_bytes = (size_t)T::CC * a.lrow * 4;
+    const size_t data_bytes = (size_t)T::CC * a.lrow * sizeof(typename T::In);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int dm_lo = blockIdx.x * T::DMS_CTA;
     const int g_lo = blockIdx.x * T::WD;
     const int T0 = blockIdx.y * T::SAMPLES_CTA;
     const int nchunks = (a.C + T::CC - 1) / T::CC;
-    const float *in = (const float *)a.in + (size_t)blockIdx.z * a.C * a.in_pitch;
+    const typename T::In *in =
+        (const typename T::In *)a.in + (size_t)blockIdx.z * a.C * a.in_pitch;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < T::NSTAGE; ++s) {
@@ -122,9 +137,37 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
         const int s = k % T::NSTAGE;
         mbar_wait(&full[s], (k / T::NSTAGE) & 1);
         const unsigned char *st = stages + (size_t)s * sbytes;
-        const float *rows = reinterpret_cast<const float *>(st) + tw + lane * T::TT;
-        const uint32_t *ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
         const int ncc = (a.C - k * T::CC) < T::CC ? (a.C - k * T::CC) : T::CC;
+        const float *rows;
+        const uint32_t *ds;
+        if constexpr (T::U8) {
+            // convert the chunk's uint8 rows to fp32 (exact; sums stay below 2^24, checked at plan
+            // creation), copy its descriptors, release the stage, meet the other warps
+            unsigned char *fb = stages + T::NSTAGE * sbytes + (size_t)(k & 1) * tree_fbuf_bytes<T>(a.lrow);
+            float4 *frow = reinterpret_cast<float4 *>(fb);
+            const uint32_t *raw = reinterpret_cast<const uint32_t *>(st);
+            const int nwords = ncc * a.lrow / 4;  // 4 samples per 32-bit word
+            for (int i = threadIdx.x; i < nwords; i += T::THREADS) {
+                const uint32_t x = raw[i];
+                // byte b -> float: 0x4B000000 | b is 2^23 + b
+                float4 v;
+                v.x = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7650)) - 8388608.f;
+                v.y = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7651)) - 8388608.f;
+                v.z = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7652)) - 8388608.f;
+                v.w = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7653)) - 8388608.f;
+                frow[i] = v;
+            }
+            uint32_t *fds = reinterpret_cast<uint32_t *>(fb + (size_t)T::CC * a.lrow * 4);
+            if ((int)threadIdx.x < ncc * T::WD)
+                fds[threadIdx.x] = reinterpret_cast<const uint32_t *>(st + data_bytes)[threadIdx.x];
+            __syncthreads();
+            if (lane == 0) mbar_arrive(&empty[s]);
+            rows = reinterpret_cast<const float *>(fb) + tw + lane * T::TT;
+            ds = fds + g;
+        } else {
+            rows = reinterpret_cast<const float *>(st) + tw + lane * T::TT;
+            ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
+        }
         uint32_t dn = __shfl_sync(0xffffffffu, ds[0], 0);  // descriptors one channel ahead
 #pragma unroll 1
         for (int cc = 0; cc < ncc; ++cc) {
@@ -135,8 +178,10 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
                                                  (int)((d >> 12) & 15u), (int)(woff & 3u),
                                                  d & 0xfffu);
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[s]);
+        if constexpr (!T::U8) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
         // producer duty, rotating over the warps (step a4): refill the stage chunk k-1 used, which
         // the other warps have normally left by now
         const int kk = k + T::NSTAGE - 1;
@@ -148,23 +193,33 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     }
 
     // store (step a6): each thread writes TT consecutive samples of each of its DMs
-    float *out = (float *)a.out + (size_t)blockIdx.z * a.D * a.S;
+    typedef typename T::Acc Acc;
+    Acc *out = (Acc *)a.out + (size_t)blockIdx.z * a.D * a.S;
     const int dm0 = dm_lo + g * T::DT;
     const int t0 = T0 + tw + lane * T::TT;
     const bool vec = (a.S & 3) == 0 && t0 + T::TT <= a.S;
 #pragma unroll
     for (int j = 0; j < T::DT; ++j) {
         if (dm0 + j >= a.D) break;
-        float *o = out + (size_t)(dm0 + j) * a.S + t0;
+        Acc *o = out + (size_t)(dm0 + j) * a.S + t0;
         if (vec) {
 #pragma unroll
-            for (int k = 0; k < T::TT; k += 4)
-                *reinterpret_cast<float4 *>(o + k) =
-                    make_float4(acc[j][k], acc[j][k + 1], acc[j][k + 2], acc[j][k + 3]);
+            for (int k = 0; k < T::TT; k += 4) {
+                if constexpr (T::U8)
+                    *reinterpret_cast<uint4 *>(o + k) =
+                        make_uint4(__float2uint_rn(acc[j][k]), __float2uint_rn(acc[j][k + 1]),
+                                   __float2uint_rn(acc[j][k + 2]), __float2uint_rn(acc[j][k + 3]));
+                else
+                    *reinterpret_cast<float4 *>(o + k) =
+                        make_float4(acc[j][k], acc[j][k + 1], acc[j][k + 2], acc[j][k + 3]);
+            }
         } else {
 #pragma unroll
             for (int k = 0; k < T::TT; ++k)
-                if (t0 + k < a.S) o[k] = acc[j][k];
+                if (t0 + k < a.S) {
+                    if constexpr (T::U8) o[k] = __float2uint_rn(acc[j][k]);
+                    else o[k] = acc[j][k];
+                }
         }
     }
 }

@@ -23,7 +23,7 @@ void register_regwin0(std::vector<Variant> &);
 void register_regwin1(std::vector<Variant> &);
 void register_regwin2(std::vector<Variant> &);
 void register_regwin3(std::vector<Variant> &);
-#define DEDISP_TREE_PARTS 12  // rows of TREE_VARIANTS in variants_tree.cu
+// one per row of TREE_VARIANTS in variants_tree.cu
 void register_tree0(std::vector<Variant> &);
 void register_tree1(std::vector<Variant> &);
 void register_tree2(std::vector<Variant> &);
@@ -36,11 +36,13 @@ void register_tree8(std::vector<Variant> &);
 void register_tree9(std::vector<Variant> &);
 void register_tree10(std::vector<Variant> &);
 void register_tree11(std::vector<Variant> &);
+void register_tree12(std::vector<Variant> &);
+void register_tree13(std::vector<Variant> &);
+void register_tree14(std::vector<Variant> &);
+void register_tree15(std::vector<Variant> &);
 void register_tree(std::vector<Variant> &r) {
-    void (*parts[DEDISP_TREE_PARTS])(std::vector<Variant> &) = {
-        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4,
-        register_tree5, register_tree6, register_tree7, register_tree8, register_tree9,
-        register_tree10, register_tree11};
+    void (*parts[])(std::vector<Variant> &) = {
+        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4, register_tree5, register_tree6, register_tree7, register_tree8, register_tree9, register_tree10, register_tree11, register_tree12, register_tree13, register_tree14, register_tree15};
     for (auto f : parts) f(r);
 }
 void register_regwin(std::vector<Variant> &r) {
@@ -131,7 +133,8 @@ static cudaError_t build_tree_tables(dedisp_plan *pl) {
             pl->tree.tables.push_back(t);  // owned by the plan from here on
             if ((e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
                 (e = build_tree_desc(pl->d_shiftT, d_qc, pl->C, pl->D, pl->dpitch, v.dt, v.dms_cta,
-                                     t.pitch, t.d_desc, d_flags, 0)) != cudaSuccess ||
+                                     pl->dtype == DEDISP_U8 ? 16 : 4, t.pitch, t.d_desc, d_flags,
+                                     0)) != cudaSuccess ||
                 (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess)
                 break;
             pl->tree.tables.back().valid = h[1] == 0;

@@ -92,13 +92,13 @@ __global__ void chan_slope_kernel(const int32_t *shiftT, int D, int dpitch, int 
 // desc_kernel: one thread per (channel c, DM group G of dt DMs); the group belongs to the CTA tile
 // of dms_cta DMs that starts at DM lo = (G*dt / dms_cta) * dms_cta.
 //   desc[c][G] = woff << 16 | q_c << 12 | bits
-//   woff = shift(c, G*dt) - (shift(c, lo) & ~3): offset of the group's first DM in the staged row,
-//          whose element 0 is input sample T0 + (shift(c, lo) & ~3);
+//   woff = shift(c, G*dt) - (shift(c, lo) & ~(al-1)): offset of the group's first DM in the staged
+//          row, whose element 0 is input sample T0 + (shift(c, lo) & ~(al-1));
 //   bits: increment j of the group = q_c + bit (j-1).
 // DMs past D (ragged last group, padding groups) continue with increment q_c: their outputs are
 // never stored and their window offsets stay inside the lattice.  flags[1] |= 1 if woff >= 2^16.
 __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, int dpitch, int dt,
-                            int dms_cta, int descpitch, uint32_t *desc, int *flags) {
+                            int dms_cta, int al, int descpitch, uint32_t *desc, int *flags) {
     int G = blockIdx.x * blockDim.x + threadIdx.x;
     int c = blockIdx.y;
     if (G >= descpitch) return;
@@ -106,7 +106,7 @@ __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, 
     const long d0 = (long)G * dt;
     const long lo = d0 / dms_cta * dms_cta;
     const int e0 = row[d0 < D ? d0 : D - 1];
-    const int base = row[lo < D ? lo : D - 1] & ~3;
+    const int base = row[lo < D ? lo : D - 1] & ~(al - 1);  // al = input elements per 16 bytes
     const int q = qc[c];
     uint32_t bits = 0;
     for (int j = 1; j < dt && d0 + j < D; ++j) {
@@ -126,11 +126,11 @@ cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch,
 }
 
 cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int D, int dpitch,
-                            int dt, int dms_cta, int descpitch, uint32_t *d_desc, int *d_flags,
-                            cudaStream_t st) {
+                            int dt, int dms_cta, int al, int descpitch, uint32_t *d_desc,
+                            int *d_flags, cudaStream_t st) {
     dim3 block(128);
     dim3 grid((descpitch + 127) / 128, C);
-    desc_kernel<<<grid, block, 0, st>>>(d_shiftT, d_qc, C, D, dpitch, dt, dms_cta, descpitch,
+    desc_kernel<<<grid, block, 0, st>>>(d_shiftT, d_qc, C, D, dpitch, dt, dms_cta, al, descpitch,
                                         d_desc, d_flags);
     return cudaGetLastError();
 }

@@ -13,8 +13,10 @@ static VariantFit tree_fit(const Variant &v, const PlanShape &p, int span_cta) {
     if (!p.tree->valid || p.tree->qmax > T::QMAX) return f;
     const TreeTable *t = p.tree->find(T::DT, T::DMS_CTA);
     if (!t || !t->valid) return f;
-    long lrow = (long)T::SAMPLES_CTA + span_cta + 8 + T::WNMAX;
-    lrow = (lrow + 3) / 4 * 4;
+    // uint8 sums are accumulated in fp32: exact while C * 255 < 2^24
+    if (T::U8 && (long)p.C * 255 >= (1L << 24)) return f;
+    long lrow = (long)T::SAMPLES_CTA + span_cta + 2 * T::AL + T::WNMAX;
+    lrow = (lrow + T::AL - 1) / T::AL * T::AL;
     size_t smem = tree_smem_bytes<T>((int)lrow);
     if (smem > kMaxSmem) return f;
     if ((p.S + T::SAMPLES_CTA - 1) / T::SAMPLES_CTA > 65535) return f;
@@ -42,11 +44,11 @@ template <typename T>
 static Variant make_tree() {
     static char name[112];
     snprintf(name, sizeof name,
-             "tree_f32: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d q%d b%d", T::DMS_CTA,
-             T::SAMPLES_CTA, T::DT, T::TT, T::CC, T::NSTAGE, T::QMAX, T::MINB);
+             "tree_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d q%d b%d",
+             T::U8 ? "u8" : "f32", T::DMS_CTA, T::SAMPLES_CTA, T::DT, T::TT, T::CC, T::NSTAGE, T::QMAX, T::MINB);
     Variant v;
     v.name = name;
-    v.dtype = DEDISP_F32;
+    v.dtype = T::U8 ? DEDISP_U8 : DEDISP_F32;
     v.kind = KIND_TREE;
     v.dms_cta = T::DMS_CTA;
     v.samples_cta = T::SAMPLES_CTA;
@@ -64,30 +66,33 @@ static Variant make_tree() {
 
 // One variant per translation unit (-DTREE_PART=i): build.py reads this list for the parts and for
 // the (DT, TT, QMAX) lattices gen_tree.py must emit.
-//        part WD WT DT TT CC NS QMAX MINB        DMs x samples per CTA
-#define TREE_VARIANTS(X)              \
-    X(0, 8, 1, 8, 20, 8, 4, 3, 1)  /* 64 x 640  */ \
-    X(1, 4, 2, 8, 20, 8, 4, 3, 1)  /* 32 x 1280 */ \
-    X(2, 8, 1, 4, 28, 8, 4, 4, 1)  /* 32 x 896  */ \
-    X(3, 12, 1, 4, 20, 8, 4, 4, 1) /* 48 x 640  */ \
-    X(4, 16, 1, 6, 12, 8, 4, 4, 1) /* 96 x 384  */ \
-    X(5, 12, 1, 8, 12, 8, 4, 4, 1) /* 96 x 384  */ \
-    X(6, 8, 1, 4, 12, 8, 3, 4, 2)  /* 32 x 384, 2 CTAs/SM */ \
-    X(7, 8, 1, 6, 20, 8, 4, 4, 1)  /* 48 x 640  */ \
-    X(8, 8, 1, 8, 20, 8, 4, 4, 1)  /* 64 x 640, q <= 4 */ \
-    X(9, 8, 2, 4, 12, 8, 4, 4, 1)  /* 32 x 768, 16 warps */ \
-    X(10, 8, 1, 4, 20, 8, 3, 4, 1) /* 32 x 640 (also 2 CTAs/SM by registers) */ \
-    X(11, 4, 1, 4, 12, 8, 3, 4, 4) /* 16 x 384, small problems */
+//    part  input   WD WT DT TT CC NS QMAX MINB        DMs x samples per CTA
+#define TREE_VARIANTS(X)                                                  \
+    X(0, float, 8, 1, 8, 20, 8, 4, 3, 1)    /* 64 x 640  */                \
+    X(1, float, 4, 2, 8, 20, 8, 4, 3, 1)    /* 32 x 1280 */                \
+    X(2, float, 8, 1, 4, 28, 8, 4, 4, 1)    /* 32 x 896  */                \
+    X(3, float, 12, 1, 4, 20, 8, 4, 4, 1)   /* 48 x 640  */                \
+    X(4, float, 16, 1, 6, 12, 8, 4, 4, 1)   /* 96 x 384  */                \
+    X(5, float, 12, 1, 8, 12, 8, 4, 4, 1)   /* 96 x 384  */                \
+    X(6, float, 8, 1, 4, 12, 8, 3, 4, 2)    /* 32 x 384, 2 CTAs/SM */      \
+    X(7, float, 8, 1, 6, 20, 8, 4, 4, 1)    /* 48 x 640  */                \
+    X(8, float, 8, 1, 8, 20, 8, 4, 4, 1)    /* 64 x 640, q <= 4 */         \
+    X(9, float, 8, 1, 6, 28, 8, 4, 3, 1)    /* 48 x 896 */                 \
+    X(10, float, 8, 1, 8, 20, 4, 6, 3, 1)   /* 64 x 640, cc4 s6 */         \
+    X(11, float, 4, 1, 4, 12, 8, 3, 4, 4)   /* 16 x 384, small problems */ \
+    X(12, uint8_t, 8, 1, 8, 20, 8, 4, 4, 1) /* 64 x 640  */                \
+    X(13, uint8_t, 16, 1, 6, 12, 8, 4, 4, 1) /* 96 x 384 */                \
+    X(14, uint8_t, 8, 1, 6, 28, 8, 4, 4, 1) /* 48 x 896  */                \
+    X(15, uint8_t, 4, 1, 4, 12, 8, 3, 4, 4) /* 16 x 384, small problems */
 
 #ifndef TREE_PART
 #define TREE_PART 0
 #endif
 #define DEDISP_CAT(a, b) a##b
 #define DEDISP_TREE_REG(P) DEDISP_CAT(register_tree, P)
-// select the part
-#define X(P, WD, WT, DT, TT, CC, NS, QMAX, MINB) \
-    template <> struct TreePart<P> { typedef TreeTile<WD, WT, DT, TT, CC, NS, QMAX, MINB> type; };
 template <int P> struct TreePart;
+#define X(P, IN, WD, WT, DT, TT, CC, NS, QMAX, MINB) \
+    template <> struct TreePart<P> { typedef TreeTile<IN, WD, WT, DT, TT, CC, NS, QMAX, MINB> type; };
 TREE_VARIANTS(X)
 #undef X
 void DEDISP_TREE_REG(TREE_PART)(std::vector<Variant> &r) {
