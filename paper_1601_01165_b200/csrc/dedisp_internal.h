@@ -58,7 +58,7 @@ struct TreeTable {
     bool valid = false;          // every woff fits 16 bits
 };
 struct TreeInfo {
-    bool valid = false;  // every channel's increments are {q_c, q_c + 1}, q_c <= 15
+    bool valid = false;  // every channel's increments are {q_c, q_c + 1}, q_c <= 7
     int qmax = -1;       // max_c q_c
     std::vector<TreeTable> tables;
     const TreeTable *find(int dt, int dms_cta) const {

@@ -13,7 +13,7 @@
 //   per thread : DT adjacent DMs x TT consecutive samples in registers.
 //   per channel: one descriptor word per (channel, DM group) built at plan creation
 //                (desc_kernel, shift_table.cu):  [31:16] window offset in the staged row
-//                [15:12] q_c   [11:0] bits, the group's shift increments being q_c + bit_j.
+//                [15:8] 1 << q_c   [7:0] bits, the group's shift increments being q_c + bit_j.
 //                Staged per chunk next to the input rows.
 #pragma once
 #include "kernels.cuh"
@@ -38,7 +38,7 @@ struct TreeTile {
     static_assert(TT % 4 == 0, "thread windows are loaded with LDS.128");
     static_assert(WD % 4 == 0, "descriptor rows are copied in 16-byte units");
     static_assert(CC <= 32, "one lane per channel of a chunk issues its copies");
-    static_assert(DT <= 13, "12 increment bits per descriptor");
+    static_assert(DT <= 9 && QMAX <= 7, "8 increment bits and a one-hot q per descriptor");
     static_assert(SAMPLES_CTA % AL == 0, "time tiles start on 16-byte boundaries of the input");
 };
 
@@ -175,8 +175,7 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             if (cc + 1 < ncc) dn = __shfl_sync(0xffffffffu, ds[(cc + 1) * T::WD], 0);
             const uint32_t woff = d >> 16;
             TreeStep<T::DT, T::TT, T::QMAX>::run(acc, rows + (size_t)cc * a.lrow + (woff & ~3u),
-                                                 (int)((d >> 12) & 15u), (int)(woff & 3u),
-                                                 d & 0xfffu);
+                                                 (d >> 8) & 0xffu, (int)(woff & 3u), d & 0xffu);
         }
         if constexpr (!T::U8) {
             __syncwarp();

@@ -80,7 +80,7 @@ __global__ void chan_slope_kernel(const int32_t *shiftT, int D, int dpitch, int 
         mn = smn[0];
         mx = smx[0];
         if (mn == 0x7fffffff) mn = 0;  // D == 1
-        if (mn < 0 || mn > 15 || mx - mn > 1) {
+        if (mn < 0 || mn > 7 || mx - mn > 1) {
             atomicOr(&flags[1], 1);
             mn = 0;
         }
@@ -91,7 +91,7 @@ __global__ void chan_slope_kernel(const int32_t *shiftT, int D, int dpitch, int 
 
 // desc_kernel: one thread per (channel c, DM group G of dt DMs); the group belongs to the CTA tile
 // of dms_cta DMs that starts at DM lo = (G*dt / dms_cta) * dms_cta.
-//   desc[c][G] = woff << 16 | q_c << 12 | bits
+//   desc[c][G] = woff << 16 | (1 << q_c) << 8 | bits          (dt <= 9, q_c <= 7)
 //   woff = shift(c, G*dt) - (shift(c, lo) & ~(al-1)): offset of the group's first DM in the staged
 //          row, whose element 0 is input sample T0 + (shift(c, lo) & ~(al-1));
 //   bits: increment j of the group = q_c + bit (j-1).
@@ -116,7 +116,7 @@ __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, 
     }
     const int woff = e0 - base;
     if (woff < 0 || woff > 0xffff) atomicOr(&flags[1], 1);
-    desc[(size_t)c * descpitch + G] = ((uint32_t)woff & 0xffffu) << 16 | (uint32_t)q << 12 | bits;
+    desc[(size_t)c * descpitch + G] = ((uint32_t)woff & 0xffffu) << 16 | (0x100u << q) | bits;
 }
 
 cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch, int *d_qc,
