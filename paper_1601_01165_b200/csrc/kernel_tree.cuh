@@ -43,8 +43,9 @@ struct TreeTile {
 };
 
 // Shared memory (dynamic): mbarriers | NSTAGE stages { CC input rows of lrow elements | CC x WD
-// descriptors } | for uint8 input two fp32 buffers { CC rows of lrow floats | CC x WD descriptors }
-// the compute loop reads (the stage rows are converted into them, chunk k into buffer k & 1).
+// descriptors } | for uint8 input three fp32 buffers { CC rows of lrow floats | CC x WD descriptors }
+// the compute loop reads (the stage rows are converted into them, chunk k into buffer k % 3, one
+// chunk ahead of the adds).
 template <typename T>
 __host__ __device__ inline size_t tree_stage_bytes(int lrow) {
     return (size_t)T::CC * ((size_t)lrow * sizeof(typename T::In) + (size_t)T::WD * 4);
@@ -55,8 +56,8 @@ __host__ __device__ inline size_t tree_fbuf_bytes(int lrow) {
 }
 template <typename T>
 __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
-    return T::NSTAGE * tree_stage_bytes<T>(lrow) + (T::U8 ? 2 * tree_fbuf_bytes<T>(lrow) : 0) +
-           2 * T::NSTAGE * sizeof(uint64_t) + 16;
+    return T::NSTAGE * tree_stage_bytes<T>(lrow) + (T::U8 ? 3 * tree_fbuf_bytes<T>(lrow) : 0) +
+           (2 * T::NSTAGE + 3) * sizeof(uint64_t) + 16;
 }
 
 // Issue the copies of chunk k into its stage (called by one whole warp; lane l < CC stages channel
@@ -99,7 +100,9 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);
     uint64_t *empty = full + T::NSTAGE;
-    unsigned char *stages = smem_raw + ((2 * T::NSTAGE * sizeof(uint64_t) + 15) & ~(size_t)15);
+    uint64_t *conv = empty + T::NSTAGE;  // uint8 input: fp32 buffer b holds a converted chunk
+    unsigned char *stages =
+        smem_raw + (((2 * T::NSTAGE + 3) * sizeof(uint64_t) + 15) & ~(size_t)15);
     const size_t sbytes = tree_stage_bytes<T>(a.lrow);
     const size_t data_bytes = (size_t)T::CC * a.lrow * sizeof(typename T::In);
 
@@ -116,12 +119,15 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], T::NW);
         }
+        for (int b = 0; b < 3; ++b) mbar_init(&conv[b], T::NW);
         mbar_fence_init();
     }
     __syncthreads();
-    // prologue: warp 0 fills the first NSTAGE-1 stages
+    // prologue: warp 0 fills the first NSTAGE-1 stages (all NSTAGE for uint8 input, whose stages
+    // are released one chunk early, after conversion)
+    constexpr int AHEAD = T::U8 ? T::NSTAGE : T::NSTAGE - 1;
     if (warp == 0)
-        for (int k = 0; k < T::NSTAGE - 1 && k < nchunks; ++k)
+        for (int k = 0; k < AHEAD && k < nchunks; ++k)
             tree_issue<T>(a, in, desc, descpitch, k, lane, T0, dm_lo, g_lo, stages, sbytes,
                           data_bytes, full);
 
@@ -133,38 +139,55 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
 #pragma unroll
         for (int k = 0; k < T::TT; ++k) acc[j][k] = 0.f;
 
-    for (int k = 0; k < nchunks; ++k) {
+    // uint8 input: convert chunk k's rows to fp32 (exact; sums stay below 2^24, checked at plan
+    // creation) into buffer k % 3, copy its descriptors, release the stage.  Every warp converts a
+    // slice; conv[k % 3] completes when all have.
+    auto convert = [&](int k) {
         const int s = k % T::NSTAGE;
         mbar_wait(&full[s], (k / T::NSTAGE) & 1);
         const unsigned char *st = stages + (size_t)s * sbytes;
         const int ncc = (a.C - k * T::CC) < T::CC ? (a.C - k * T::CC) : T::CC;
+        unsigned char *fb = stages + T::NSTAGE * sbytes + (size_t)(k % 3) * tree_fbuf_bytes<T>(a.lrow);
+        float4 *frow = reinterpret_cast<float4 *>(fb);
+        const uint32_t *raw = reinterpret_cast<const uint32_t *>(st);
+        const int nwords = ncc * a.lrow / 4;  // 4 samples per 32-bit word
+        for (int i = threadIdx.x; i < nwords; i += T::THREADS) {
+            const uint32_t x = raw[i];
+            float4 v;  // byte b -> float: 0x4B000000 | b is 2^23 + b
+            v.x = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7650)) - 8388608.f;
+            v.y = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7651)) - 8388608.f;
+            v.z = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7652)) - 8388608.f;
+            v.w = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7653)) - 8388608.f;
+            frow[i] = v;
+        }
+        uint32_t *fds = reinterpret_cast<uint32_t *>(fb + (size_t)T::CC * a.lrow * 4);
+        if ((int)threadIdx.x < ncc * T::WD)
+            fds[threadIdx.x] = reinterpret_cast<const uint32_t *>(st + data_bytes)[threadIdx.x];
+        __syncwarp();
+        if (lane == 0) {
+            mbar_arrive(&conv[k % 3]);
+            mbar_arrive(&empty[s]);
+        }
+    };
+    if constexpr (T::U8) convert(0);
+
+    for (int k = 0; k < nchunks; ++k) {
+        const int s = k % T::NSTAGE;
+        const int ncc = (a.C - k * T::CC) < T::CC ? (a.C - k * T::CC) : T::CC;
         const float *rows;
         const uint32_t *ds;
         if constexpr (T::U8) {
-            // convert the chunk's uint8 rows to fp32 (exact; sums stay below 2^24, checked at plan
-            // creation), copy its descriptors, release the stage, meet the other warps
-            unsigned char *fb = stages + T::NSTAGE * sbytes + (size_t)(k & 1) * tree_fbuf_bytes<T>(a.lrow);
-            float4 *frow = reinterpret_cast<float4 *>(fb);
-            const uint32_t *raw = reinterpret_cast<const uint32_t *>(st);
-            const int nwords = ncc * a.lrow / 4;  // 4 samples per 32-bit word
-            for (int i = threadIdx.x; i < nwords; i += T::THREADS) {
-                const uint32_t x = raw[i];
-                // byte b -> float: 0x4B000000 | b is 2^23 + b
-                float4 v;
-                v.x = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7650)) - 8388608.f;
-                v.y = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7651)) - 8388608.f;
-                v.z = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7652)) - 8388608.f;
-                v.w = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7653)) - 8388608.f;
-                frow[i] = v;
-            }
-            uint32_t *fds = reinterpret_cast<uint32_t *>(fb + (size_t)T::CC * a.lrow * 4);
-            if ((int)threadIdx.x < ncc * T::WD)
-                fds[threadIdx.x] = reinterpret_cast<const uint32_t *>(st + data_bytes)[threadIdx.x];
-            __syncthreads();
-            if (lane == 0) mbar_arrive(&empty[s]);
+            // all warps have converted chunk k, so all have finished the adds of chunk k-2, whose
+            // buffer chunk k+1 is converted into now
+            mbar_wait(&conv[k % 3], (k / 3) & 1);
+            if (k + 1 < nchunks) convert(k + 1);
+            const unsigned char *fb =
+                stages + T::NSTAGE * sbytes + (size_t)(k % 3) * tree_fbuf_bytes<T>(a.lrow);
             rows = reinterpret_cast<const float *>(fb) + tw + lane * T::TT;
-            ds = fds + g;
+            ds = reinterpret_cast<const uint32_t *>(fb + (size_t)T::CC * a.lrow * 4) + g;
         } else {
+            mbar_wait(&full[s], (k / T::NSTAGE) & 1);
+            const unsigned char *st = stages + (size_t)s * sbytes;
             rows = reinterpret_cast<const float *>(st) + tw + lane * T::TT;
             ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
         }
@@ -181,9 +204,9 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);
         }
-        // producer duty, rotating over the warps (step a4): refill the stage chunk k-1 used, which
-        // the other warps have normally left by now
-        const int kk = k + T::NSTAGE - 1;
+        // producer duty, rotating over the warps (step a4): refill the most recently released
+        // stage, which the other warps have normally left by now
+        const int kk = k + AHEAD;
         if (kk < nchunks && warp == k % T::NW) {
             if (kk >= T::NSTAGE) mbar_wait(&empty[kk % T::NSTAGE], ((kk / T::NSTAGE) - 1) & 1);
             tree_issue<T>(a, in, desc, descpitch, kk, lane, T0, dm_lo, g_lo, stages, sbytes,
