@@ -35,7 +35,10 @@ FALLBACK_HBM_GBS = 6650.0        # B200_PROFILING.md fallback
 FALLBACK_SM_MHZ = 1965.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the
 # same command (profiles/README.md says which file); None until captured for that config.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r01_ncu_tree_apertif.md: 114.8 MB read + 123.9 MB written per launch
+    "apertif": 114810112 + 123915520,
+}
 
 
 def measured_peaks():
