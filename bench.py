@@ -107,6 +107,22 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(x: float, world: int, device="cuda") -> float:
+    """Replicas only: the one cross-rank step is taking the slowest rank's time."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(adds_per_rank: int, world: int, seconds_max: float) -> float:
+    """Whole-job GFLOP/s: every rank processed the same number of adds (weak scaling)."""
+    return world * adds_per_rank / seconds_max / 1e9
+
+
 def cpu_baseline(s, target_s: float = 12.0):
     """The oracle as it stands, on this box's host cores, on a bounded sample of the workload: a
     subset of DM rows at full C and S (each output is still the full channel sum)."""
@@ -261,10 +277,7 @@ def run_ours(args, s):
     total_ms = ev[0].elapsed_time(ev[-1])
     per = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps))
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world)
     ms_step = total_ms / args.steps
 
     # ---- end to end through the host-buffer entry point (pinned host memory)
@@ -279,13 +292,10 @@ def run_ours(args, s):
         plan.execute_host(h_in, h_out, nr_beams=B, stream=stream)   # synchronises the stream
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world)
 
     adds = B * D * C * S
-    value = world * adds / (ms_step * 1e-3) / 1e9
+    value = aggregate_value(adds, world, ms_step * 1e-3)
     secs = S / s.sample_rate
     rt = secs / (ms_step * 1e-3 / B)
     if rank == 0:
@@ -315,7 +325,7 @@ def run_ours(args, s):
                              "peak_gbs": hbm_gbs, "peak_kind": peak_kind,
                              "frac": comp / (kern_ms * 1e-3) / 1e9 / hbm_gbs,
                              "frac_of_nominal_8TBs": comp / (kern_ms * 1e-3) / 8e12},
-            "e2e": {"value": world * adds / e2e_s / 1e9, "unit": UNIT,
+            "e2e": {"value": aggregate_value(adds, world, e2e_s), "unit": UNIT,
                     "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
                     "d2h_bytes_per_step": h_out.numel() * h_out.element_size(),
                     "ms_per_step": e2e_s * 1e3},

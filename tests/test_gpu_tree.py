@@ -1,0 +1,94 @@
+"""KIND_TREE kernels (kernel_tree.cuh): which plans get them, and parity where the slope classes,
+the ragged DM groups and the staging ring are stressed."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1601_01165_b200 import workloads as wl
+from test_gpu_parity import check_full, dd, make_case, out_buffer, to_host  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def tree_variants(dd, plan):
+    return [v for v in plan.supported_variants() if dd.variant_name(v).startswith("tree_")]
+
+
+def max_q(table):
+    """largest per-channel minimum increment (the q_c of DESIGN.md section 5), from the oracle table"""
+    if table.shape[0] < 2:
+        return 0
+    return int(np.diff(table.astype(np.int64), axis=0).min(axis=0).max())
+
+
+@pytest.mark.parametrize("name,expect", [("tiny", True), ("apertif", True), ("survey8", True),
+                                         ("batch40", True), ("lofar", False)])
+def test_which_configs_get_tree_kernels(dd, name, expect):
+    s = wl.CONFIGS[name]
+    with dd.Plan(*s.plan_args()) as plan:
+        tv = tree_variants(dd, plan)
+        assert bool(tv) == expect
+        table = oracle.shift_table(*s.table_args())
+        inc = np.diff(table.astype(np.int64), axis=0)
+        ok = bool(((inc.max(axis=0) - inc.min(axis=0)) <= 1).all())
+        assert ok  # every BASELINE table is a rounded linear function of the DM index
+        for v in tv:  # a variant is only offered when its lattice covers the plan's slope classes
+            qcap = int(dd.variant_name(v).split(" q")[1].split()[0])
+            assert qcap >= max_q(table)
+        if name == "lofar":
+            assert max_q(table) > 7
+
+
+def run_tree(dd, setup, exact):
+    plan, table, x, d_in = make_case(dd, setup)
+    ref, sabs = oracle.dedisperse(x, table, setup.nr_samples, want_sabs=True)
+    tv = tree_variants(dd, plan)
+    for v in tv:
+        d_out = out_buffer(setup, fill=-1 if setup.in_dtype == wl.U8 else float("nan"))
+        plan.execute_variant(v, d_in, d_out, nr_beams=setup.nr_beams)
+        try:
+            check_full(setup, to_host(setup, d_out), ref, sabs, exact)
+        except AssertionError as e:
+            raise AssertionError("%s on %s: %s" % (dd.variant_name(v), setup.name, e))
+    plan.destroy()
+    return len(tv), max_q(table)
+
+
+def test_slope_class_4_only_runs_q4_lattices(dd):
+    # survey8 band, lowest channels: q_c reaches 4; integer data -> bit-exact
+    s = wl.scaled(wl.SURVEY8, name="q4_f32", nr_channels=96, channel_bw_MHz=300.0 / 96, nr_dms=131,
+                  nr_samples=2900, in_dtype=wl.F32, values="int16")
+    n, q = run_tree(dd, s, exact=True)
+    assert q == 4 and n >= 3
+    s8 = wl.scaled(wl.SURVEY8, name="q4_u8", nr_channels=96, channel_bw_MHz=300.0 / 96, nr_dms=131,
+                   nr_samples=2900)
+    n, q = run_tree(dd, s8, exact=True)
+    assert q == 4 and n >= 3
+
+
+def test_slope_beyond_the_lattice_falls_back_to_other_kinds(dd):
+    s = wl.scaled(wl.SURVEY8, name="q9", nr_channels=64, channel_bw_MHz=300.0 / 64, nr_dms=40,
+                  nr_samples=1500, dm_step=0.5, in_dtype=wl.F32, values="int16")
+    with dd.Plan(*s.plan_args()) as plan:
+        assert max_q(oracle.shift_table(*s.table_args())) > 4
+        assert not tree_variants(dd, plan)
+        assert plan.supported_variants()  # lds / generic still run it
+
+
+def test_many_chunks_ragged_everything_bit_exact(dd):
+    # 37 chunks of 8 channels + a ragged one, DMs not a multiple of 4/6/8, samples not a tile multiple
+    s = wl.scaled(wl.APERTIF, name="ring", nr_channels=301, channel_bw_MHz=300.0 / 301, nr_dms=157,
+                  nr_samples=2051, values="int16")
+    n, _ = run_tree(dd, s, exact=True)
+    assert n >= 8
+    s8 = wl.scaled(wl.SURVEY8, name="ring_u8", nr_channels=301, channel_bw_MHz=300.0 / 301,
+                   nr_dms=157, nr_samples=2064)
+    n, _ = run_tree(dd, s8, exact=True)
+    assert n >= 3
+
+
+def test_shipped_winner_for_apertif_is_a_tree_kernel(dd):
+    from paper_1601_01165_b200 import tuning
+    with dd.Plan(*wl.APERTIF.plan_args()) as plan:
+        tuning.apply_shipped(plan)
+        assert dd.variant_name(plan.variant).startswith("tree_f32")
