@@ -24,10 +24,6 @@ UNITS = [
     ("variants_generic.cu", "variants_generic.o", []),
     ("variants_lds.cu", "variants_lds.o", []),
     ("variants_u8.cu", "variants_u8.o", []),
-    ("variants_regwin.cu", "variants_regwin0.o", ["-DREGWIN_PART=0"]),
-    ("variants_regwin.cu", "variants_regwin1.o", ["-DREGWIN_PART=1"]),
-    ("variants_regwin.cu", "variants_regwin2.o", ["-DREGWIN_PART=2"]),
-    ("variants_regwin.cu", "variants_regwin3.o", ["-DREGWIN_PART=3"]),
 ]
 
 

@@ -15,7 +15,6 @@ namespace dedisp {
 enum Kind {
     KIND_GENERIC = 0,  // one (DM, sample) per thread, global-memory reads (PAPER.md:173 baseline)
     KIND_LDS = 1,      // CTA tile staged in shared memory, one shared-memory word per add
-    KIND_REGWIN = 2,   // staged tile + per-thread register window reused across the thread's DMs
     KIND_TREE = 3      // register window, offsets selected by a generated branch lattice
 };
 
@@ -77,7 +76,7 @@ struct Variant {
     int dt, tt;       // outputs per thread: dt DMs x tt samples
     int cc;           // channel-chunk depth (channels per pipeline stage)
     int stages;
-    int rstep;        // REGWIN: largest per-DM-step shift increment the switch covers
+    int rstep;        // KIND_TREE: largest slope class q_c the variant's lattice covers (QMAX)
     int threads;
     // Fills lrow/smem, returns whether the variant supports the plan.
     VariantFit (*fit)(const Variant &, const PlanShape &, int span_cta);
@@ -89,7 +88,6 @@ const std::vector<Variant> &variants();
 // Each variants_*.cu appends its instantiations.
 void register_generic(std::vector<Variant> &);
 void register_lds(std::vector<Variant> &);
-void register_regwin(std::vector<Variant> &);
 void register_u8(std::vector<Variant> &);
 void register_tree(std::vector<Variant> &);
 

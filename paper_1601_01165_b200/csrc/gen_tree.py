@@ -11,7 +11,8 @@ plans that violate it do not get this kernel).  The thread loads the window
 w[0 .. WN_q) = row[a0 .. a0 + WN_q) once (LDS.128, a0 16-byte aligned) and DM j adds
 w[R_j + k], k < TT, with R_0 = m0 = (e_0 - row origin) & 3 and R_j = R_{j-1} + q + b_j.  m0, q and
 the bits b_j are warp-uniform, so the selection is a walk through nodes N[q][j][R] joined by uniform
-two-way branches: one test per DM, no indirect jump, no dynamic register index.
+two-way branches: one test per DM, no indirect jump, no dynamic register index.  Per (DT, TT, QMAX)
+the generator emits one lattice function per q and the channel loop of a staged chunk around them.
 
 Usage: python gen_tree.py OUT.cuh DT,TT,QMAX [DT,TT,QMAX ...]
 """
@@ -30,36 +31,60 @@ def emit(dt: int, tt: int, qmax: int) -> str:
     wnmax = wn(dt, tt, qmax)
     o.append("template <> struct TreeStep<%d, %d, %d> {" % (dt, tt, qmax))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
-    o.append("    // p: 16-byte aligned window start in shared memory; qhot (1 << q), m0, bits: warp-uniform")
-    o.append("    static __device__ __forceinline__ void run(float (&acc)[%d][%d], const float *p, "
-             "unsigned qhot, int m0, unsigned bits) {" % (dt, tt))
-    o.append("        float w[%d];" % wnmax)
-    o.append("        float4 v;")
-    o.append("        const float4 *p4 = reinterpret_cast<const float4 *>(p);")
-    # q dispatch on a one-hot mask (bit q set): single-bit tests stay compare-and-branch, where a
-    # chain of q == k tests with five or more cases is turned into an indirect jump through a
-    # constant-memory table (LDC + BRX), which costs more than the adds of a DM
-    for q in range(qmax):
-        o.append("        if (qhot & %du) goto Q%d;" % (1 << q, q))
-    o.append("        goto Q%d;" % qmax)
+    # one lattice per slope class q
     for q in range(qmax + 1):
-        n4 = wn(dt, tt, q) // 4
-        o.append("    Q%d:" % q)
-        for m in range(n4):
+        n = wn(dt, tt, q)
+        o.append("    // slope class q = %d.  p: 16-byte aligned window start in shared memory; m0, bits: "
+                 "warp-uniform" % q)
+        o.append("    static __device__ __forceinline__ void run_q%d(float (&acc)[%d][%d], const float *p, "
+                 "unsigned m0, unsigned bits) {" % (q, dt, tt))
+        o.append("        float w[%d];" % n)
+        o.append("        float4 v;")
+        o.append("        const float4 *p4 = reinterpret_cast<const float4 *>(p);")
+        for m in range(n // 4):
             o.append("        v = p4[%d]; w[%d] = v.x; w[%d] = v.y; w[%d] = v.z; w[%d] = v.w;"
                      % (m, 4 * m, 4 * m + 1, 4 * m + 2, 4 * m + 3))
-        o.append("        if (m0 & 2) { if (m0 & 1) goto Q%d_0_3; else goto Q%d_0_2; }" % (q, q))
-        o.append("        else { if (m0 & 1) goto Q%d_0_1; else goto Q%d_0_0; }" % (q, q))
+        o.append("        if (m0 & 2u) { if (m0 & 1u) goto N_0_3; else goto N_0_2; }")
+        o.append("        else { if (m0 & 1u) goto N_0_1; else goto N_0_0; }")
         for j in range(dt):
             for r in range(j * q, j * q + 3 + j + 1):
-                o.append("    Q%d_%d_%d:" % (q, j, r))
+                o.append("    N_%d_%d:" % (j, r))
                 o.append("        tree_add<%d, %d>(acc[%d], w);" % (r, tt, j))
                 if j + 1 < dt:
-                    o.append("        if (bits & %du) goto Q%d_%d_%d; else goto Q%d_%d_%d;"
-                             % (1 << j, q, j + 1, r + q + 1, q, j + 1, r + q))
+                    o.append("        if (bits & %du) goto N_%d_%d; else goto N_%d_%d;"
+                             % (1 << j, j + 1, r + q + 1, j + 1, r + q))
                 else:
                     o.append("        goto DONE;")
-    o.append("    DONE:;")
+        o.append("    DONE:;")
+        o.append("    }")
+    # the channel loop of one staged chunk.  The slope class is tested only when it changes: channels
+    # are ordered by frequency, so q_c is constant over long runs.  Testing single bits of a one-hot
+    # mask keeps the dispatch compare-and-branch (a chain of q == k tests with five or more cases is
+    # turned into an indirect jump through a constant-memory table, LDC + BRX).
+    o.append("    // rows: the thread's position in channel 0's staged row; ds: the warp's descriptor of")
+    o.append("    // channel 0 (stride wd words per channel); descriptors are broadcast with SHFL so that the")
+    o.append("    // compiler knows they are warp-uniform, one channel ahead of their use")
+    o.append("    static __device__ __forceinline__ void chunk(float (&acc)[%d][%d], const float *rows, "
+             "const uint32_t *ds, int ncc, int lrow, int wd) {" % (dt, tt))
+    o.append("        uint32_t d = __shfl_sync(0xffffffffu, ds[0], 0), dn;")
+    o.append("        int cc = 0;")
+    o.append("    NEXT:")
+    for q in range(qmax):
+        o.append("        if (d & %du) goto L%d;" % (0x100 << q, q))
+    o.append("        goto L%d;" % qmax)
+    for q in range(qmax + 1):
+        o.append("    L%d:" % q)
+        o.append("        do {")
+        o.append("            dn = d;")
+        o.append("            if (cc + 1 < ncc) dn = __shfl_sync(0xffffffffu, ds[(cc + 1) * wd], 0);")
+        o.append("            run_q%d(acc, rows + (size_t)cc * lrow + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);"
+                 % q)
+        o.append("            d = dn;")
+        o.append("            ++cc;")
+        o.append("        } while (cc < ncc && (d & %du));" % (0x100 << q))
+        o.append("        if (cc < ncc) goto NEXT;")
+        o.append("        goto END;")
+    o.append("    END:;")
     o.append("    }")
     o.append("};")
     return "\n".join(o)
@@ -67,6 +92,7 @@ def emit(dt: int, tt: int, qmax: int) -> str:
 
 HEADER = """// GENERATED by gen_tree.py -- do not edit.  KIND_TREE add lattices (see gen_tree.py).
 #pragma once
+#include <stdint.h>
 namespace dedisp {
 template <int DT, int TT, int QMAX> struct TreeStep;
 // acc[k] += w[R + k], all indices static.  Inline asm keeps the optimiser from merging the add

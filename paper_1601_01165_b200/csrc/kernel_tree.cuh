@@ -191,15 +191,7 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             rows = reinterpret_cast<const float *>(st) + tw + lane * T::TT;
             ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
         }
-        uint32_t dn = __shfl_sync(0xffffffffu, ds[0], 0);  // descriptors one channel ahead
-#pragma unroll 1
-        for (int cc = 0; cc < ncc; ++cc) {
-            const uint32_t d = dn;
-            if (cc + 1 < ncc) dn = __shfl_sync(0xffffffffu, ds[(cc + 1) * T::WD], 0);
-            const uint32_t woff = d >> 16;
-            TreeStep<T::DT, T::TT, T::QMAX>::run(acc, rows + (size_t)cc * a.lrow + (woff & ~3u),
-                                                 (d >> 8) & 0xffu, (int)(woff & 3u), d & 0xffu);
-        }
+        TreeStep<T::DT, T::TT, T::QMAX>::chunk(acc, rows, ds, ncc, a.lrow, T::WD);
         if constexpr (!T::U8) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);

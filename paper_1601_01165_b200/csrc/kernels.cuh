@@ -8,12 +8,9 @@
 //                    into shared memory with 1-D bulk async copies (cp.async.bulk, SASS UBLKCP)
 //                    completing on an mbarrier ring; consumer warps accumulate DT x TT outputs
 //                    per thread in registers (work-items computing several
-//                    elements, data reuse through local memory).  Two inner loops:
-//                      KIND_LDS    one shared-memory word per add, lanes on consecutive samples;
-//                      KIND_REGWIN each thread owns TT consecutive samples, loads the window that
-//                                  covers all its DT DMs once (LDS.128) and reuses it from
-//                                  registers; the warp-uniform offset of each DM inside the
-//                                  window selects a statically indexed add block.
+//                    elements, data reuse through local memory), one shared-memory word per add,
+//                    lanes on consecutive samples (KIND_LDS).
+// The register-window kernels (KIND_TREE) are in kernel_tree.cuh.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -89,7 +86,7 @@ __global__ void __launch_bounds__(256) generic_kernel(KArgs a) {
 // ---------------------------------------------------------------- tiled kernels
 // Compile-time tile description.
 //   WD x WT consumer warps: WD DM groups of DT DMs, WT time chunks of 32*TT samples.
-//   CC channels per pipeline stage, NSTAGE stages, RSTEP see KIND_REGWIN.
+//   CC channels per pipeline stage, NSTAGE stages (RSTEP_ is unused, kept for the variant tables).
 template <typename In_, int KIND_, int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_,
           int RSTEP_, int MINB_>
 struct Tile {
@@ -102,9 +99,6 @@ struct Tile {
     static constexpr int DMS_CTA = WD * DT;
     static constexpr int SAMPLES_CTA = WT * 32 * TT;
     static constexpr int AL = 16 / (int)sizeof(In);  // elements per 16 bytes
-    // REGWIN: offset of DM j inside the thread's window is at most 3 + RSTEP*j.
-    static constexpr int RMAX = 3 + RSTEP * (DT - 1);
-    static constexpr int WN = ((RMAX + TT + 3) / 4) * 4;  // window registers
     static_assert(DMS_CTA % 4 == 0, "shift rows are copied in 16-byte units");
     static_assert(CC <= 32, "one producer lane per channel of a chunk");
 };
@@ -120,41 +114,6 @@ __host__ __device__ inline size_t tile_smem_bytes(int lrow) {
     return T::NSTAGE * stage_bytes<T>(lrow) + 2 * T::NSTAGE * sizeof(uint64_t) + 16;
 }
 
-// ---- REGWIN add blocks: acc[k] += w[R + k], all indices static.
-template <int R, int TT, int WN>
-__device__ __forceinline__ void add_block(float (&acc)[TT], const float (&w)[WN]) {
-    if constexpr (R + TT <= WN) {
-#pragma unroll
-        for (int k = 0; k < TT; ++k) acc[k] += w[R + k];
-    }
-}
-// Select the add block for the warp-uniform offset r in [0, RJ].
-#define DEDISP_CASE(R)                                      \
-    case R:                                                 \
-        if constexpr (R <= RJ) add_block<R, TT, WN>(acc, w); \
-        break;
-template <int RJ, int TT, int WN>
-__device__ __forceinline__ void add_select(int r, float (&acc)[TT], const float (&w)[WN]) {
-    static_assert(RJ < 64, "offset range of the switch");
-    switch (r) {
-        DEDISP_CASE(0) DEDISP_CASE(1) DEDISP_CASE(2) DEDISP_CASE(3) DEDISP_CASE(4) DEDISP_CASE(5)
-        DEDISP_CASE(6) DEDISP_CASE(7) DEDISP_CASE(8) DEDISP_CASE(9) DEDISP_CASE(10)
-        DEDISP_CASE(11) DEDISP_CASE(12) DEDISP_CASE(13) DEDISP_CASE(14) DEDISP_CASE(15)
-        DEDISP_CASE(16) DEDISP_CASE(17) DEDISP_CASE(18) DEDISP_CASE(19) DEDISP_CASE(20)
-        DEDISP_CASE(21) DEDISP_CASE(22) DEDISP_CASE(23) DEDISP_CASE(24) DEDISP_CASE(25)
-        DEDISP_CASE(26) DEDISP_CASE(27) DEDISP_CASE(28) DEDISP_CASE(29) DEDISP_CASE(30)
-        DEDISP_CASE(31) DEDISP_CASE(32) DEDISP_CASE(33) DEDISP_CASE(34) DEDISP_CASE(35)
-        DEDISP_CASE(36) DEDISP_CASE(37) DEDISP_CASE(38) DEDISP_CASE(39) DEDISP_CASE(40)
-        DEDISP_CASE(41) DEDISP_CASE(42) DEDISP_CASE(43) DEDISP_CASE(44) DEDISP_CASE(45)
-        DEDISP_CASE(46) DEDISP_CASE(47) DEDISP_CASE(48) DEDISP_CASE(49) DEDISP_CASE(50)
-        DEDISP_CASE(51) DEDISP_CASE(52) DEDISP_CASE(53) DEDISP_CASE(54) DEDISP_CASE(55)
-        DEDISP_CASE(56) DEDISP_CASE(57) DEDISP_CASE(58) DEDISP_CASE(59) DEDISP_CASE(60)
-        DEDISP_CASE(61) DEDISP_CASE(62) DEDISP_CASE(63)
-        default: break;
-    }
-}
-#undef DEDISP_CASE
-
 // ---- per-channel inner loops -------------------------------------------------------------
 // row : the channel's staged span; element 0 is input sample T0 + (smin & ~(AL-1)) where smin is
 //       the shift of the CTA's first DM.  sh : the channel's DMS_CTA shifts (shared memory).
@@ -169,52 +128,6 @@ __device__ __forceinline__ void channel_lds(typename T::Acc (&acc)[T::DT][T::TT]
 #pragma unroll
         for (int k = 0; k < T::TT; ++k) acc[j][k] += (typename T::Acc)p[32 * k];
     }
-}
-
-// Compile-time loop over the thread's DMs: DM j's offset is at most 3 + RSTEP*j, so its switch
-// only carries that many add blocks.
-template <typename T, int J>
-__device__ __forceinline__ void dm_loop(const int (&e)[T::DT], int off, float (&acc)[T::DT][T::TT],
-                                        const float (&w)[T::WN]) {
-    add_select<3 + T::RSTEP * J, T::TT, T::WN>(e[J] - off, acc[J], w);
-    if constexpr (J + 1 < T::DT) dm_loop<T, J + 1>(e, off, acc, w);
-}
-
-template <typename T>
-__device__ __forceinline__ void channel_regwin(float (&acc)[T::DT][T::TT], const float *row,
-                                               const int32_t *sh, int g, int tw, int lane) {
-    static_assert(T::TT % 4 == 0, "thread windows are loaded with LDS.128");
-    const int base = sh[0] & ~3;
-    int e[T::DT];
-    if constexpr (T::DT % 4 == 0) {
-#pragma unroll
-        for (int j = 0; j < T::DT; j += 4) {
-            int4 v = *reinterpret_cast<const int4 *>(sh + g * T::DT + j);
-            e[j] = v.x; e[j + 1] = v.y; e[j + 2] = v.z; e[j + 3] = v.w;
-        }
-    } else if constexpr (T::DT % 2 == 0) {
-#pragma unroll
-        for (int j = 0; j < T::DT; j += 2) {
-            int2 v = *reinterpret_cast<const int2 *>(sh + g * T::DT + j);
-            e[j] = v.x; e[j + 1] = v.y;
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j < T::DT; ++j) e[j] = sh[g * T::DT + j];
-    }
-    const int a0 = (e[0] - base) & ~3;          // window start, 16-byte aligned
-    const int off = base + a0;                   // e[j] - off = offset of DM j in the window
-    const int nW = (e[T::DT - 1] - off + T::TT + 3) >> 2;  // 16-byte chunks actually needed
-    const float4 *p = reinterpret_cast<const float4 *>(row + tw + lane * T::TT + a0);
-    float w[T::WN];
-#pragma unroll
-    for (int m = 0; m < T::WN / 4; ++m) {
-        if (m < (T::TT + 3) / 4 || m < nW) {  // the first chunks are always needed
-            float4 v = p[m];
-            w[4 * m] = v.x; w[4 * m + 1] = v.y; w[4 * m + 2] = v.z; w[4 * m + 3] = v.w;
-        }
-    }
-    dm_loop<T, 0>(e, off, acc, w);
 }
 
 // ---- the tiled kernel --------------------------------------------------------------------
@@ -295,22 +208,12 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tiled_kernel(KArgs a) {
         if (ncc == T::CC) {
 #pragma unroll 1
             for (int cc = 0; cc < T::CC; ++cc) {
-                if constexpr (T::KIND == KIND_REGWIN)
-                    channel_regwin<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g,
-                                      tw, lane);
-                else
-                    channel_lds<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g, tw,
-                                   lane);
+                channel_lds<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g, tw, lane);
             }
         } else {
 #pragma unroll 1
             for (int cc = 0; cc < ncc; ++cc) {
-                if constexpr (T::KIND == KIND_REGWIN)
-                    channel_regwin<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g,
-                                      tw, lane);
-                else
-                    channel_lds<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g, tw,
-                                   lane);
+                channel_lds<T>(acc, rows + (size_t)cc * a.lrow, shs + cc * T::DMS_CTA, g, tw, lane);
             }
         }
         __syncwarp();
@@ -320,34 +223,14 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tiled_kernel(KArgs a) {
     // ---------------- store (step a6): aligned, contiguous per thread / per warp
     Acc *out = (Acc *)a.out + (size_t)blockIdx.z * a.D * a.S;
     const int dm0 = dm_lo + g * T::DT;
-    if constexpr (T::KIND == KIND_REGWIN) {
-        const int t0 = T0 + tw + lane * T::TT;
-        const bool vec = (a.S & 3) == 0 && t0 + T::TT <= a.S;
+    const int t0 = T0 + tw + lane;
 #pragma unroll
-        for (int j = 0; j < T::DT; ++j) {
-            if (dm0 + j >= a.D) break;
-            Acc *o = out + (size_t)(dm0 + j) * a.S + t0;
-            if (vec) {
+    for (int j = 0; j < T::DT; ++j) {
+        if (dm0 + j >= a.D) break;
+        Acc *o = out + (size_t)(dm0 + j) * a.S + t0;
 #pragma unroll
-                for (int k = 0; k < T::TT; k += 4)
-                    *reinterpret_cast<float4 *>(o + k) =
-                        make_float4(acc[j][k], acc[j][k + 1], acc[j][k + 2], acc[j][k + 3]);
-            } else {
-#pragma unroll
-                for (int k = 0; k < T::TT; ++k)
-                    if (t0 + k < a.S) o[k] = acc[j][k];
-            }
-        }
-    } else {
-        const int t0 = T0 + tw + lane;
-#pragma unroll
-        for (int j = 0; j < T::DT; ++j) {
-            if (dm0 + j >= a.D) break;
-            Acc *o = out + (size_t)(dm0 + j) * a.S + t0;
-#pragma unroll
-            for (int k = 0; k < T::TT; ++k)
-                if (t0 + 32 * k < a.S) o[32 * k] = acc[j][k];
-        }
+        for (int k = 0; k < T::TT; ++k)
+            if (t0 + 32 * k < a.S) o[32 * k] = acc[j][k];
     }
 }
 

@@ -19,10 +19,6 @@ void set_last_error(const char *what, cudaError_t e) {
     snprintf(g_last_error, sizeof g_last_error, "%s: %s", what, cudaGetErrorString(e));
 }
 
-void register_regwin0(std::vector<Variant> &);
-void register_regwin1(std::vector<Variant> &);
-void register_regwin2(std::vector<Variant> &);
-void register_regwin3(std::vector<Variant> &);
 // one per row of TREE_VARIANTS in variants_tree.cu
 void register_tree0(std::vector<Variant> &);
 void register_tree1(std::vector<Variant> &);
@@ -40,16 +36,17 @@ void register_tree12(std::vector<Variant> &);
 void register_tree13(std::vector<Variant> &);
 void register_tree14(std::vector<Variant> &);
 void register_tree15(std::vector<Variant> &);
+void register_tree16(std::vector<Variant> &);
+void register_tree17(std::vector<Variant> &);
+void register_tree18(std::vector<Variant> &);
+void register_tree19(std::vector<Variant> &);
+void register_tree20(std::vector<Variant> &);
+void register_tree21(std::vector<Variant> &);
 void register_tree(std::vector<Variant> &r) {
     void (*parts[])(std::vector<Variant> &) = {
-        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4, register_tree5, register_tree6, register_tree7, register_tree8, register_tree9, register_tree10, register_tree11, register_tree12, register_tree13, register_tree14, register_tree15};
+        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4, register_tree5, register_tree6, register_tree7, register_tree8, register_tree9, register_tree10, register_tree11, register_tree12, register_tree13, register_tree14, register_tree15, register_tree16, register_tree17, register_tree18, register_tree19,
+        register_tree20, register_tree21};
     for (auto f : parts) f(r);
-}
-void register_regwin(std::vector<Variant> &r) {
-    register_regwin0(r);
-    register_regwin1(r);
-    register_regwin2(r);
-    register_regwin3(r);
 }
 
 const std::vector<Variant> &variants() {
@@ -59,7 +56,6 @@ const std::vector<Variant> &variants() {
         register_generic(reg);  // variants 0 (f32) and 1 (u8): the no-reuse baseline
         register_lds(reg);
         register_u8(reg);
-        register_regwin(reg);
         register_tree(reg);
     });
     return reg;
@@ -154,7 +150,7 @@ static int heuristic_variant(const dedisp_plan *pl) {
     for (size_t v = 0; v < vs.size(); ++v) {
         if (!pl->fit[v].ok) continue;
         const Variant &x = vs[v];
-        double rate = x.kind == KIND_TREE ? 2.0 : x.kind == KIND_REGWIN ? 0.8 : x.kind == KIND_LDS ? 1.0 : 0.25;
+        double rate = x.kind == KIND_TREE ? 2.0 : x.kind == KIND_LDS ? 1.0 : 0.25;
         double nd = std::ceil((double)pl->D / x.dms_cta), nt = std::ceil((double)pl->S / x.samples_cta);
         double work = nd * x.dms_cta * nt * x.samples_cta;  // padded outputs
         double ctas = nd * nt;

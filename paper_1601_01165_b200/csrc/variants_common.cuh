@@ -13,8 +13,7 @@ template <typename T>
 VariantFit tiled_fit(const Variant &v, const PlanShape &p, int span_cta) {
     VariantFit f;
     if (p.dtype != v.dtype) return f;
-    if (T::KIND == KIND_REGWIN && p.max_step > T::RSTEP) return f;
-    long lrow = (long)T::SAMPLES_CTA + span_cta + 2 * T::AL + (T::KIND == KIND_REGWIN ? T::WN : 0);
+    long lrow = (long)T::SAMPLES_CTA + span_cta + 2 * T::AL + 0;
     lrow = (lrow + T::AL - 1) / T::AL * T::AL;
     size_t smem = tile_smem_bytes<T>((int)lrow);
     if (smem > kMaxSmem) return f;
@@ -39,19 +38,13 @@ cudaError_t tiled_prepare(size_t smem) {
                                 (int)smem);
 }
 
-// name: "<kind>_<dtype> DMSxSAMPLES dtxtt ccN sN [rN]" -- kept in static storage.
+// name: "lds_<dtype>: DMSxSAMPLES DMsxsamples/CTA, dtxtt outputs/thread, ccN sN bN" (static storage).
 template <typename T>
 Variant make_tiled() {
     static char name[96];
-    const char *kind = T::KIND == KIND_REGWIN ? "regwin" : "lds";
     const char *dt = sizeof(typename T::In) == 1 ? "u8" : "f32";
-    if (T::KIND == KIND_REGWIN)
-        snprintf(name, sizeof name, "%s_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d r%d b%d",
-                 kind, dt, T::DMS_CTA, T::SAMPLES_CTA, T::DT, T::TT, T::CC, T::NSTAGE, T::RSTEP,
-                 T::MINB);
-    else
-        snprintf(name, sizeof name, "%s_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d b%d",
-                 kind, dt, T::DMS_CTA, T::SAMPLES_CTA, T::DT, T::TT, T::CC, T::NSTAGE, T::MINB);
+    snprintf(name, sizeof name, "lds_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d b%d", dt,
+             T::DMS_CTA, T::SAMPLES_CTA, T::DT, T::TT, T::CC, T::NSTAGE, T::MINB);
     Variant v;
     v.name = name;
     v.dtype = sizeof(typename T::In) == 1 ? DEDISP_U8 : DEDISP_F32;
@@ -62,7 +55,7 @@ Variant make_tiled() {
     v.tt = T::TT;
     v.cc = T::CC;
     v.stages = T::NSTAGE;
-    v.rstep = T::KIND == KIND_REGWIN ? T::RSTEP : 0;
+    v.rstep = 0;
     v.threads = T::THREADS;
     v.fit = tiled_fit<T>;
     v.launch = tiled_launch<T>;

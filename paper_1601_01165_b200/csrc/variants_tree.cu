@@ -83,7 +83,13 @@ static Variant make_tree() {
     X(12, uint8_t, 8, 1, 8, 20, 8, 4, 4, 1) /* 64 x 640  */                \
     X(13, uint8_t, 16, 1, 6, 12, 8, 4, 4, 1) /* 96 x 384 */                \
     X(14, uint8_t, 8, 1, 6, 28, 8, 4, 4, 1) /* 48 x 896  */                \
-    X(15, uint8_t, 4, 1, 4, 12, 8, 3, 4, 4) /* 16 x 384, small problems */
+    X(15, uint8_t, 4, 1, 4, 12, 8, 3, 4, 4) /* 16 x 384, small problems */ \
+    X(16, float, 12, 1, 4, 28, 8, 4, 3, 1)  /* 48 x 896, 12 warps */       \
+    X(17, float, 8, 1, 5, 36, 8, 4, 3, 1)   /* 40 x 1152 */                \
+    X(18, float, 8, 1, 4, 44, 8, 3, 3, 1)   /* 32 x 1408 */                \
+    X(19, float, 12, 1, 5, 20, 8, 4, 3, 1)  /* 60 x 640, 12 warps */       \
+    X(20, float, 8, 1, 6, 28, 16, 2, 3, 1)  /* 48 x 896, cc16 s2 */        \
+    X(21, float, 8, 1, 6, 28, 4, 6, 3, 1)   /* 48 x 896, cc4 s6 */
 
 #ifndef TREE_PART
 #define TREE_PART 0

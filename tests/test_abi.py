@@ -49,7 +49,7 @@ def test_variant_registry_is_readable_without_a_gpu(lib_path):
     assert len(set(names)) == n, "variant names are the tuning-cache keys: must be unique"
     assert names[0].startswith("generic_f32") and names[1].startswith("generic_u8")
     assert dedisp.variant_name(n) is None and dedisp.variant_name(-1) is None
-    assert any(s.startswith("regwin_f32") for s in names)
+    assert any(s.startswith("tree_f32") for s in names) and any(s.startswith("tree_u8") for s in names)
     assert any(s.startswith("lds_u8") for s in names)
 
 

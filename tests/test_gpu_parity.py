@@ -104,7 +104,7 @@ def test_tiny_every_variant_bit_exact_and_pulse(dd):
         got = to_host(s, d_out)
         assert np.array_equal(got.astype(np.float64), ref), dd.variant_name(v)
         ran.append(dd.variant_name(v))
-    assert any(n.startswith("regwin") for n in ran) and any(n.startswith("lds") for n in ran)
+    assert any(n.startswith("tree") for n in ran) and any(n.startswith("lds") for n in ran)
     # the default (heuristic or tuned) launch, and the injected pulse (readings A13/A14)
     d_out = out_buffer(s, fill=-1.0)
     plan.execute(d_in, d_out)
