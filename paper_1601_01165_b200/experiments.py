@@ -1,0 +1,94 @@
+"""The paper's experiments on the current GPU, as markdown tables.
+
+  python -m paper_1601_01165_b200.experiments [sweep] [zerodm] [histogram]
+
+sweep     PAPER.md:105-107, Figs. 1-2: the two Table 2 setups (Apertif 1024 ch / 20 kHz / 1420 MHz / 300 MHz,
+          LOFAR 32 ch / 200 kHz / 138 MHz / 6 MHz), trial DMs from 0 in steps of 0.25, 12 instances from 2 to
+          4096 DMs, each auto-tuned (dedisp_tune) as in the paper; GFLOP/s, the winner, the real-time factor,
+          and the speed-up over the no-reuse "generically tuned" kernel (Fig. 4).
+zerodm    PAPER.md:157-169 (section 4.3): all trial DMs equal to 0, i.e. perfect data reuse.
+histogram PAPER.md:151, Fig. 3: the distribution of GFLOP/s over the whole tuning space (every compiled variant).
+
+Inputs are zeros of the right shape (values do not affect timing); parity is the tests' business.
+"""
+from __future__ import annotations
+
+import sys
+
+import numpy as np
+
+from . import dedisp, workloads as wl
+
+PAPER_APERTIF = wl.Setup("apertif-paper", 1024, 1420.0, 300.0 / 1024, 20000.0, 20000, 0.0, 0.25, 2)
+PAPER_LOFAR = wl.Setup("lofar-paper", 32, 138.0, 6.0 / 32, 200000.0, 200000, 0.0, 0.25, 2)
+DM_COUNTS = [2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096]
+
+
+def tune_once(setup):
+    """plan + zero buffers + dedisp_tune -> ({variant: ms}, plan facts)."""
+    import torch
+    plan = dedisp.Plan(*setup.plan_args())
+    in_dt = torch.uint8 if setup.in_dtype == wl.U8 else torch.float32
+    d_in = torch.zeros((1, setup.nr_channels, plan.in_pitch), dtype=in_dt, device="cuda")
+    d_out = torch.empty((1, setup.nr_dms, setup.nr_samples), dtype=torch.float32, device="cuda")
+    ms = plan.tune(d_in, d_out)
+    facts = {"max_shift": plan.max_shift, "winner": dedisp.variant_name(plan.variant)}
+    plan.destroy()
+    del d_in, d_out
+    torch.cuda.empty_cache()
+    return ms, facts
+
+
+def gflops(setup, ms):
+    return setup.adds_per_beam / (ms * 1e-3) / 1e9
+
+
+def short(name):
+    return name.split(" DMsxsamples")[0] + "," + name.split("CTA,")[1].split(" outputs")[0]
+
+
+def sweep():
+    print("| setup | DMs | max shift | GFLOP/s | ms | real-time factor | winner | generic GFLOP/s | tuned / generic |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    for base in (PAPER_APERTIF, PAPER_LOFAR):
+        for d in DM_COUNTS:
+            s = wl.scaled(base, nr_dms=d)
+            ms, facts = tune_once(s)
+            best = min(ms.values())
+            generic = ms[0]  # variant 0 = generic_f32
+            print("| %s | %d | %d | %.0f | %.4f | %.0f | %s | %.0f | %.1fx |"
+                  % (base.name, d, facts["max_shift"], gflops(s, best), best,
+                     s.seconds_of_data / (best * 1e-3), short(facts["winner"]), gflops(s, generic),
+                     generic / best), flush=True)
+
+
+def zerodm():
+    print("| setup | DMs | GFLOP/s, all DMs = 0 (perfect reuse) | winner | GFLOP/s, step 0.25 | winner |")
+    print("|---|---|---|---|---|---|")
+    for base in (PAPER_APERTIF, PAPER_LOFAR):
+        for d in (256, 2048):
+            z = wl.scaled(base, nr_dms=d, dm_step=0.0)
+            r = wl.scaled(base, nr_dms=d)
+            msz, fz = tune_once(z)
+            msr, fr = tune_once(r)
+            print("| %s | %d | %.0f | %s | %.0f | %s |"
+                  % (base.name, d, gflops(z, min(msz.values())), short(fz["winner"]),
+                     gflops(r, min(msr.values())), short(fr["winner"])), flush=True)
+
+
+def histogram():
+    for s in (wl.APERTIF, wl.LOFAR, wl.SURVEY8):
+        ms, facts = tune_once(s)
+        g = np.array(sorted(gflops(s, t) for t in ms.values()))
+        print("\n%s: %d variants, GFLOP/s min %.0f / median %.0f / max %.0f (winner %s)"
+              % (s.name, len(g), g[0], np.median(g), g[-1], short(facts["winner"])))
+        edges = np.linspace(0, g[-1] * 1.0001, 11)
+        hist, _ = np.histogram(g, bins=edges)
+        for lo, hi, n in zip(edges[:-1], edges[1:], hist):
+            print("  %7.0f - %7.0f GFLOP/s | %s %d" % (lo, hi, "#" * int(n), n))
+
+
+if __name__ == "__main__":
+    what = sys.argv[1:] or ["sweep", "zerodm", "histogram"]
+    for w in what:
+        {"sweep": sweep, "zerodm": zerodm, "histogram": histogram}[w]()
