@@ -89,7 +89,11 @@ static Variant make_tree() {
     X(18, float, 8, 1, 4, 44, 8, 3, 3, 1)   /* 32 x 1408 */                \
     X(19, float, 12, 1, 5, 20, 8, 4, 3, 1)  /* 60 x 640, 12 warps */       \
     X(20, float, 8, 1, 6, 28, 16, 2, 3, 1)  /* 48 x 896, cc16 s2 */        \
-    X(21, float, 8, 1, 6, 28, 4, 6, 3, 1)   /* 48 x 896, cc4 s6 */
+    X(21, float, 8, 1, 6, 28, 4, 6, 3, 1)   /* 48 x 896, cc4 s6 */         \
+    X(22, uint8_t, 12, 1, 4, 20, 8, 4, 4, 1) /* 48 x 640, 12 warps */      \
+    X(23, uint8_t, 12, 1, 4, 28, 8, 4, 3, 1) /* 48 x 896, 12 warps, q <= 3 */ \
+    X(24, uint8_t, 8, 1, 8, 20, 8, 4, 3, 1)  /* 64 x 640, q <= 3 */        \
+    X(25, uint8_t, 16, 1, 4, 12, 8, 4, 4, 1) /* 64 x 384, 16 warps */
 
 #ifndef TREE_PART
 #define TREE_PART 0
