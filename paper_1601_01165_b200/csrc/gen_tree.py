@@ -76,8 +76,8 @@ def emit(dt: int, tt: int, qmax: int) -> str:
         o.append("        do {")
         o.append("            dn = d;")
         o.append("            if (cc + 1 < ncc) dn = tree_desc(ds + (cc + 1) * wd);")
-        o.append("            run_q%d(acc, rows + (size_t)cc * lrow + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);"
-                 % q)
+        o.append("            run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q)
+        o.append("            rows += lrow;")
         o.append("            d = dn;")
         o.append("            ++cc;")
         o.append("        } while (cc < ncc && (d & %du));" % (0x100 << q))
