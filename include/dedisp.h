@@ -124,6 +124,22 @@ int dedisp_execute_variant(const dedisp_plan *plan, int variant, const void *d_i
 int dedisp_execute_host(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams,
                         void *stream);
 
+/*
+ * dedisp_execute_host_async / dedisp_host_sync -- dedisp_execute_host as a pipeline: the call
+ * enqueues H2D copy, kernels and D2H copy on three plan-owned streams over three plan-owned device
+ * workspaces (allocated or grown on demand) and returns WITHOUT synchronising, so that consecutive
+ * calls overlap the upload of one batch, the kernels of the previous and the download of the one
+ * before (the streaming, real-time use the paper targets).  h_in / h_out as in
+ * dedisp_execute_host; they must be page-locked for the copies to be asynchronous and must stay
+ * valid, and h_in unmodified, until dedisp_host_sync returns (or until three later calls on the
+ * plan have been made and synchronised).  Results of call n are complete in h_out after
+ * dedisp_host_sync.  Calls on one plan must come from one thread at a time.  dedisp_plan_destroy
+ * synchronises and frees the pipeline.
+ * Errors: INVALID_ARG, ALLOC (workspaces), CUDA.
+ */
+int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams);
+int dedisp_host_sync(dedisp_plan *plan);
+
 /* dedisp_plan_destroy -- frees the plan's host and device tables.  NULL is a no-op. */
 int dedisp_plan_destroy(dedisp_plan *plan);
 

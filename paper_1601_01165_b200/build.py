@@ -21,6 +21,7 @@ UNITS = [
     ("shift_table.cu", "shift_table.o", []),
     ("plan.cu", "plan.o", []),
     ("tuner.cu", "tuner.o", []),
+    ("host_pipe.cu", "host_pipe.o", []),
     ("variants_generic.cu", "variants_generic.o", []),
     ("variants_lds.cu", "variants_lds.o", []),
     ("variants_u8.cu", "variants_u8.o", []),

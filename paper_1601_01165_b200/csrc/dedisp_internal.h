@@ -104,6 +104,18 @@ cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int
 
 void set_last_error(const char *what, cudaError_t e);
 
+// Three-stage host pipeline of dedisp_execute_host_async (host_pipe.cu).
+struct HostPipe {
+    static constexpr int kSlots = 3;
+    bool ready = false;
+    cudaStream_t s_h2d = nullptr, s_exec = nullptr, s_d2h = nullptr;
+    void *in[kSlots] = {}, *out[kSlots] = {};
+    cudaEvent_t ev_in[kSlots] = {}, ev_exec[kSlots] = {}, ev_out[kSlots] = {};
+    size_t in_bytes = 0, out_bytes = 0;
+    uint64_t calls = 0;
+    void destroy();
+};
+
 }  // namespace dedisp
 
 struct dedisp_plan {
@@ -121,4 +133,5 @@ struct dedisp_plan {
     // host-buffer path workspace (dedisp_execute_host)
     void *ws_in = nullptr, *ws_out = nullptr;
     size_t ws_in_bytes = 0, ws_out_bytes = 0;
+    dedisp::HostPipe pipe;  // dedisp_execute_host_async
 };

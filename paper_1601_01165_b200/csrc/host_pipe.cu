@@ -1,0 +1,129 @@
+// host_pipe.cu -- dedisp_execute_host_async / dedisp_host_sync: the end-to-end path for HOST buffers
+// as a three-stage pipeline.  The paper keeps data resident on the device because dedispersion is
+// one stage of a longer real-time pipeline; when the samples do come from
+// the host, consecutive calls overlap: the H2D copy of call n+1, the kernel of call n and the D2H
+// copy of call n-1 run on three streams over kSlots device workspaces, ordered by events.
+#include <cstdio>
+
+#include "dedisp_internal.h"
+
+using namespace dedisp;
+
+extern "C" int dedisp_execute(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
+                              void *stream);
+
+namespace dedisp {
+
+void HostPipe::destroy() {
+    for (int i = 0; i < kSlots; ++i) {
+        if (in[i]) cudaFree(in[i]);
+        if (out[i]) cudaFree(out[i]);
+        if (ev_in[i]) cudaEventDestroy(ev_in[i]);
+        if (ev_exec[i]) cudaEventDestroy(ev_exec[i]);
+        if (ev_out[i]) cudaEventDestroy(ev_out[i]);
+        in[i] = out[i] = nullptr;
+        ev_in[i] = ev_exec[i] = ev_out[i] = nullptr;
+    }
+    if (s_h2d) cudaStreamDestroy(s_h2d);
+    if (s_exec) cudaStreamDestroy(s_exec);
+    if (s_d2h) cudaStreamDestroy(s_d2h);
+    s_h2d = s_exec = s_d2h = nullptr;
+    in_bytes = out_bytes = 0;
+    ready = false;
+}
+
+// Streams and events once; workspaces grown (after draining the pipeline) when a call needs more.
+static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
+    cudaError_t e = cudaSuccess;
+    if (!p.ready) {
+        if ((e = cudaStreamCreateWithFlags(&p.s_h2d, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&p.s_exec, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaStreamCreateWithFlags(&p.s_d2h, cudaStreamNonBlocking)) != cudaSuccess) {
+            set_last_error("cudaStreamCreate", e);
+            return DEDISP_ERR_CUDA;
+        }
+        for (int i = 0; i < HostPipe::kSlots; ++i)
+            if ((e = cudaEventCreateWithFlags(&p.ev_in[i], cudaEventDisableTiming)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&p.ev_exec[i], cudaEventDisableTiming)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&p.ev_out[i], cudaEventDisableTiming)) != cudaSuccess) {
+                set_last_error("cudaEventCreate", e);
+                return DEDISP_ERR_CUDA;
+            }
+        p.ready = true;
+    }
+    if (in_bytes > p.in_bytes || out_bytes > p.out_bytes) {
+        cudaStreamSynchronize(p.s_h2d);
+        cudaStreamSynchronize(p.s_exec);
+        cudaStreamSynchronize(p.s_d2h);
+        for (int i = 0; i < HostPipe::kSlots; ++i) {
+            if (in_bytes > p.in_bytes) {
+                if (p.in[i]) cudaFree(p.in[i]);
+                p.in[i] = nullptr;
+                if ((e = cudaMalloc(&p.in[i], in_bytes)) != cudaSuccess) break;
+            }
+            if (out_bytes > p.out_bytes) {
+                if (p.out[i]) cudaFree(p.out[i]);
+                p.out[i] = nullptr;
+                if ((e = cudaMalloc(&p.out[i], out_bytes)) != cudaSuccess) break;
+            }
+        }
+        if (e != cudaSuccess) {
+            set_last_error("cudaMalloc(host pipeline workspace)", e);
+            p.in_bytes = p.out_bytes = 0;
+            return DEDISP_ERR_ALLOC;
+        }
+        if (in_bytes > p.in_bytes) p.in_bytes = in_bytes;
+        if (out_bytes > p.out_bytes) p.out_bytes = out_bytes;
+    }
+    return DEDISP_OK;
+}
+
+}  // namespace dedisp
+
+#define PIPE_TRY(expr, what)                   \
+    do {                                       \
+        cudaError_t e_ = (expr);               \
+        if (e_ != cudaSuccess) {               \
+            set_last_error(what, e_);          \
+            return DEDISP_ERR_CUDA;            \
+        }                                      \
+    } while (0)
+
+extern "C" int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, void *h_out,
+                                         int nr_beams) {
+    if (!plan || !h_in || !h_out || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
+    const size_t in_bytes =
+        (size_t)nr_beams * plan->C * plan->in_pitch * (plan->dtype == DEDISP_U8 ? 1 : 4);
+    const size_t out_bytes = (size_t)nr_beams * plan->D * plan->S * 4;
+    HostPipe &p = plan->pipe;
+    int rc = pipe_prepare(p, in_bytes, out_bytes);
+    if (rc != DEDISP_OK) return rc;
+    const int s = (int)(p.calls % HostPipe::kSlots);
+    const bool reused = p.calls >= (uint64_t)HostPipe::kSlots;
+    // stage 1: H2D into slot s once the kernel that last read this slot's input has finished
+    if (reused) PIPE_TRY(cudaStreamWaitEvent(p.s_h2d, p.ev_exec[s], 0), "cudaStreamWaitEvent");
+    PIPE_TRY(cudaMemcpyAsync(p.in[s], h_in, in_bytes, cudaMemcpyHostToDevice, p.s_h2d), "H2D");
+    PIPE_TRY(cudaEventRecord(p.ev_in[s], p.s_h2d), "cudaEventRecord");
+    // stage 2: the kernels, once the input is there and the slot's previous output has left
+    PIPE_TRY(cudaStreamWaitEvent(p.s_exec, p.ev_in[s], 0), "cudaStreamWaitEvent");
+    if (reused) PIPE_TRY(cudaStreamWaitEvent(p.s_exec, p.ev_out[s], 0), "cudaStreamWaitEvent");
+    rc = dedisp_execute(plan, p.in[s], p.out[s], nr_beams, p.s_exec);
+    if (rc != DEDISP_OK) return rc;
+    PIPE_TRY(cudaEventRecord(p.ev_exec[s], p.s_exec), "cudaEventRecord");
+    // stage 3: D2H
+    PIPE_TRY(cudaStreamWaitEvent(p.s_d2h, p.ev_exec[s], 0), "cudaStreamWaitEvent");
+    PIPE_TRY(cudaMemcpyAsync(h_out, p.out[s], out_bytes, cudaMemcpyDeviceToHost, p.s_d2h), "D2H");
+    PIPE_TRY(cudaEventRecord(p.ev_out[s], p.s_d2h), "cudaEventRecord");
+    ++p.calls;
+    return DEDISP_OK;
+}
+
+extern "C" int dedisp_host_sync(dedisp_plan *plan) {
+    if (!plan) return DEDISP_ERR_INVALID_ARG;
+    HostPipe &p = plan->pipe;
+    if (!p.ready) return DEDISP_OK;
+    PIPE_TRY(cudaStreamSynchronize(p.s_h2d), "cudaStreamSynchronize");
+    PIPE_TRY(cudaStreamSynchronize(p.s_exec), "cudaStreamSynchronize");
+    PIPE_TRY(cudaStreamSynchronize(p.s_d2h), "cudaStreamSynchronize");
+    return DEDISP_OK;
+}

@@ -106,14 +106,9 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     const size_t sbytes = tree_stage_bytes<T>(a.lrow);
     const size_t data_bytes = (size_t)T::CC * a.lrow * sizeof(typename T::In);
 
-    // The warp index is read through inline asm so that the compiler's divergence analysis (which
-    // only knows CTA-wide uniformity and treats %tid as divergent) takes everything derived from it
-    // -- the warp's DM group, its descriptors, every lattice test -- as uniform and emits bra.uni:
-    // plain branches without reconvergence bookkeeping.  These values are warp-uniform, which is all
-    // bra.uni requires; lane-dependent code below uses threadIdx.x as usual.
-    unsigned tid_w;
-    asm("mov.u32 %0, %%tid.x;" : "=r"(tid_w));
-    const int warp = tid_w >> 5, lane = threadIdx.x & 31;
+    // Everything derived from the warp index -- the warp's DM group, its descriptors, every lattice
+    // test -- is warp-uniform: the lattice branches never diverge.
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int dm_lo = blockIdx.x * T::DMS_CTA;
     const int g_lo = blockIdx.x * T::WD;
     const int T0 = blockIdx.y * T::SAMPLES_CTA;

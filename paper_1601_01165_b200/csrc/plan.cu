@@ -375,6 +375,7 @@ int dedisp_plan_destroy(dedisp_plan *plan) {
         if (t.d_desc) cudaFree(t.d_desc);
     if (plan->ws_in) cudaFree(plan->ws_in);
     if (plan->ws_out) cudaFree(plan->ws_out);
+    plan->pipe.destroy();
     delete plan;
     return DEDISP_OK;
 }

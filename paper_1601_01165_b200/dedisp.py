@@ -23,7 +23,8 @@ F32, U8 = 0, 1
 # every symbol include/dedisp.h declares
 SYMBOLS = [
     "dedisp_plan_create", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
-    "dedisp_execute_variant", "dedisp_execute_host", "dedisp_plan_destroy", "dedisp_variant_count",
+    "dedisp_execute_variant", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
+    "dedisp_plan_destroy", "dedisp_variant_count",
     "dedisp_variant_name", "dedisp_variant_supported", "dedisp_plan_set_variant", "dedisp_tune",
     "dedisp_plan_load_tuning", "dedisp_status_string", "dedisp_last_error",
 ]
@@ -53,6 +54,8 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_execute.argtypes = [vp, vp, vp, ci, vp]
     lib.dedisp_execute_variant.argtypes = [vp, ci, vp, vp, ci, vp]
     lib.dedisp_execute_host.argtypes = [vp, vp, vp, ci, vp]
+    lib.dedisp_execute_host_async.argtypes = [vp, vp, vp, ci]
+    lib.dedisp_host_sync.argtypes = [vp]
     lib.dedisp_plan_destroy.argtypes = [vp]
     lib.dedisp_variant_count.argtypes = []
     lib.dedisp_variant_name.argtypes = [ci]
@@ -169,6 +172,14 @@ class Plan:
     def execute_host(self, h_in, h_out, nr_beams: int = 1, stream=None):
         _check(self._lib.dedisp_execute_host(self._h, _addr(h_in), _addr(h_out), int(nr_beams),
                                              _stream(stream)), "dedisp_execute_host")
+
+    def execute_host_async(self, h_in, h_out, nr_beams: int = 1):
+        """Enqueue H2D + kernels + D2H on the plan's three-stream pipeline; see host_sync()."""
+        _check(self._lib.dedisp_execute_host_async(self._h, _addr(h_in), _addr(h_out), int(nr_beams)),
+               "dedisp_execute_host_async")
+
+    def host_sync(self):
+        _check(self._lib.dedisp_host_sync(self._h), "dedisp_host_sync")
 
     # -- variants and tuning
     def variant_supported(self, v: int) -> bool:
