@@ -1,0 +1,72 @@
+"""Host logic of the KIND_TREE kernels: the generated add lattice (csrc/gen_tree.py).  The walk
+through the generated labels must visit, for every slope class q, window misalignment m0 and increment
+bits, exactly the nodes (j, R_j) with R_0 = m0 and R_j = R_{j-1} + q + bit_j, and
+every node must stay inside the window the class loads."""
+import importlib.util
+import itertools
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+spec = importlib.util.spec_from_file_location(
+    "gen_tree", os.path.join(ROOT, "paper_1601_01165_b200", "csrc", "gen_tree.py"))
+gen_tree = importlib.util.module_from_spec(spec)
+spec.loader.exec_module(gen_tree)
+
+
+def parse_lattice(text, q):
+    """{label: (j, r, {bit value: next label})} of run_q<q>, and its window length."""
+    body = text.split("void run_q%d(" % q)[1].split("DONE:;")[0]
+    wlen = int(re.search(r"float w\[(\d+)\];", body).group(1))
+    loads = len(re.findall(r"v = p4\[\d+\];", body))
+    assert loads * 4 == wlen
+    nodes = {}
+    for m in re.finditer(r"N_(\d+)_(\d+):\s*\n\s*tree_add<(\d+), (\d+)>\(acc\[(\d+)\], w\);\s*\n\s*(.*)", body):
+        j, r, radd, tt, jacc, tail = int(m[1]), int(m[2]), int(m[3]), int(m[4]), int(m[5]), m[6]
+        assert r == radd and j == jacc
+        t = re.match(r"if \(bits & (\d+)u\) goto (N_\d+_\d+); else goto (N_\d+_\d+);", tail)
+        if t:
+            assert int(t[1]) == 1 << j
+            nodes["N_%d_%d" % (j, r)] = (j, r, tt, {1: t[2], 0: t[3]})
+        else:
+            assert tail.startswith("goto DONE;")
+            nodes["N_%d_%d" % (j, r)] = (j, r, tt, None)
+    entry = re.search(r"if \(m0 & 2u\) \{ if \(m0 & 1u\) goto (\w+); else goto (\w+); \}\s*\n\s*"
+                      r"else \{ if \(m0 & 1u\) goto (\w+); else goto (\w+); \}", body)
+    return nodes, wlen, {3: entry[1], 2: entry[2], 1: entry[3], 0: entry[4]}
+
+
+@pytest.mark.parametrize("dt,tt,qmax", [(4, 28, 3), (6, 28, 4), (8, 20, 3), (4, 12, 4)])
+def test_lattice_walk_visits_the_right_offsets(dt, tt, qmax):
+    text = gen_tree.emit(dt, tt, qmax)
+    assert "WNMAX = %d" % gen_tree.wn(dt, tt, qmax) in text
+    for q in range(qmax + 1):
+        nodes, wlen, entry = parse_lattice(text, q)
+        assert wlen == gen_tree.wn(dt, tt, q)
+        for m0 in range(4):
+            for bits in itertools.product((0, 1), repeat=dt - 1):
+                label, r_expect = entry[m0], m0
+                for j in range(dt):
+                    jn, r, ttn, nxt = nodes[label]
+                    assert (jn, r, ttn) == (j, r_expect, tt)
+                    assert r + tt <= wlen                      # the add block stays inside the window
+                    if j + 1 < dt:
+                        label = nxt[bits[j]]
+                        r_expect += q + bits[j]
+                    else:
+                        assert nxt is None
+        # no unreachable or missing nodes: exactly (4 + j) offsets per level
+        for j in range(dt):
+            assert sorted(r for (jj, r, _, _) in nodes.values() if jj == j) == \
+                list(range(j * q, j * q + 4 + j))
+
+
+def test_chunk_loop_dispatches_one_hot_slope_classes():
+    text = gen_tree.emit(4, 28, 3)
+    chunk = text.split("void chunk(")[1]
+    for q in range(3):
+        assert "if (d & %du) goto L%d;" % (0x100 << q, q) in chunk
+        assert "run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q in chunk
+    assert "goto L3;" in chunk
