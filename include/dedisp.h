@@ -140,6 +140,21 @@ int dedisp_execute_host(dedisp_plan *plan, const void *h_in, void *h_out, int nr
 int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams);
 int dedisp_host_sync(dedisp_plan *plan);
 
+/*
+ * dedisp_stream_block_async -- streaming operation on one beam's long time series (SURVEY.md 8(f)
+ * row 4; the paper's real-time setting): dedisperse the block of nr_samples output
+ * samples that starts at sample t0, through the same pipeline as dedisp_execute_host_async.
+ *   h_series: HOST, [nr_channels][series_pitch] elements; columns [t0, t0 + S + M) of every row are
+ *             read, so consecutive blocks (t0 += S) share their last / first M input samples: nothing
+ *             is carried over on the device.
+ *   h_out   : HOST, [nr_dms][out_pitch] of float / uint32_t; columns [t0, t0 + S) of every row are
+ *             written: out[i][t] = sum_c series[c][t + shift(c, dm_i)] for t in the block.
+ * Both page-locked and valid until dedisp_host_sync.  The copies are strided (2-D) DMA transfers.
+ * Errors: INVALID_ARG (null, t0 < 0, series_pitch < t0 + S + M, out_pitch < t0 + S), ALLOC, CUDA.
+ */
+int dedisp_stream_block_async(dedisp_plan *plan, const void *h_series, int64_t series_pitch,
+                              void *h_out, int64_t out_pitch, int64_t t0);
+
 /* dedisp_plan_destroy -- frees the plan's host and device tables.  NULL is a no-op. */
 int dedisp_plan_destroy(dedisp_plan *plan);
 

@@ -89,11 +89,14 @@ static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
         }                                      \
     } while (0)
 
-extern "C" int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, void *h_out,
-                                         int nr_beams) {
-    if (!plan || !h_in || !h_out || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
-    const size_t in_bytes =
-        (size_t)nr_beams * plan->C * plan->in_pitch * (plan->dtype == DEDISP_U8 ? 1 : 4);
+// One pipelined call.  series_pitch == 0: dense batch [nr_beams][C][in_pitch] -> [nr_beams][D][S].
+// Otherwise one beam taken from / written to long host arrays: input rows of S+M samples at column
+// t0 of rows series_pitch elements apart, output rows of S samples at column t0 of rows out_pitch
+// elements apart (2-D copies).
+static int pipe_call(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams,
+                     int64_t series_pitch, int64_t out_pitch, int64_t t0) {
+    const size_t esz = plan->dtype == DEDISP_U8 ? 1 : 4;
+    const size_t in_bytes = (size_t)nr_beams * plan->C * plan->in_pitch * esz;
     const size_t out_bytes = (size_t)nr_beams * plan->D * plan->S * 4;
     HostPipe &p = plan->pipe;
     int rc = pipe_prepare(p, in_bytes, out_bytes);
@@ -102,7 +105,13 @@ extern "C" int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, vo
     const bool reused = p.calls >= (uint64_t)HostPipe::kSlots;
     // stage 1: H2D into slot s once the kernel that last read this slot's input has finished
     if (reused) PIPE_TRY(cudaStreamWaitEvent(p.s_h2d, p.ev_exec[s], 0), "cudaStreamWaitEvent");
-    PIPE_TRY(cudaMemcpyAsync(p.in[s], h_in, in_bytes, cudaMemcpyHostToDevice, p.s_h2d), "H2D");
+    if (series_pitch == 0)
+        PIPE_TRY(cudaMemcpyAsync(p.in[s], h_in, in_bytes, cudaMemcpyHostToDevice, p.s_h2d), "H2D");
+    else
+        PIPE_TRY(cudaMemcpy2DAsync(p.in[s], (size_t)plan->in_pitch * esz,
+                                   (const char *)h_in + (size_t)t0 * esz, (size_t)series_pitch * esz,
+                                   (size_t)(plan->S + plan->M) * esz, (size_t)plan->C,
+                                   cudaMemcpyHostToDevice, p.s_h2d), "H2D (2-D)");
     PIPE_TRY(cudaEventRecord(p.ev_in[s], p.s_h2d), "cudaEventRecord");
     // stage 2: the kernels, once the input is there and the slot's previous output has left
     PIPE_TRY(cudaStreamWaitEvent(p.s_exec, p.ev_in[s], 0), "cudaStreamWaitEvent");
@@ -112,10 +121,30 @@ extern "C" int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, vo
     PIPE_TRY(cudaEventRecord(p.ev_exec[s], p.s_exec), "cudaEventRecord");
     // stage 3: D2H
     PIPE_TRY(cudaStreamWaitEvent(p.s_d2h, p.ev_exec[s], 0), "cudaStreamWaitEvent");
-    PIPE_TRY(cudaMemcpyAsync(h_out, p.out[s], out_bytes, cudaMemcpyDeviceToHost, p.s_d2h), "D2H");
+    if (series_pitch == 0)
+        PIPE_TRY(cudaMemcpyAsync(h_out, p.out[s], out_bytes, cudaMemcpyDeviceToHost, p.s_d2h), "D2H");
+    else
+        PIPE_TRY(cudaMemcpy2DAsync((char *)h_out + (size_t)t0 * 4, (size_t)out_pitch * 4, p.out[s],
+                                   (size_t)plan->S * 4, (size_t)plan->S * 4, (size_t)plan->D,
+                                   cudaMemcpyDeviceToHost, p.s_d2h), "D2H (2-D)");
     PIPE_TRY(cudaEventRecord(p.ev_out[s], p.s_d2h), "cudaEventRecord");
     ++p.calls;
     return DEDISP_OK;
+}
+
+extern "C" int dedisp_execute_host_async(dedisp_plan *plan, const void *h_in, void *h_out,
+                                         int nr_beams) {
+    if (!plan || !h_in || !h_out || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
+    return pipe_call(plan, h_in, h_out, nr_beams, 0, 0, 0);
+}
+
+extern "C" int dedisp_stream_block_async(dedisp_plan *plan, const void *h_series,
+                                         int64_t series_pitch, void *h_out, int64_t out_pitch,
+                                         int64_t t0) {
+    if (!plan || !h_series || !h_out || t0 < 0 || series_pitch < t0 + plan->S + plan->M ||
+        out_pitch < t0 + plan->S)
+        return DEDISP_ERR_INVALID_ARG;
+    return pipe_call(plan, h_series, h_out, 1, series_pitch, out_pitch, t0);
 }
 
 extern "C" int dedisp_host_sync(dedisp_plan *plan) {

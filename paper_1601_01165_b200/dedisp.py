@@ -24,6 +24,7 @@ F32, U8 = 0, 1
 SYMBOLS = [
     "dedisp_plan_create", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
     "dedisp_execute_variant", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
+    "dedisp_stream_block_async",
     "dedisp_plan_destroy", "dedisp_variant_count",
     "dedisp_variant_name", "dedisp_variant_supported", "dedisp_plan_set_variant", "dedisp_tune",
     "dedisp_plan_load_tuning", "dedisp_status_string", "dedisp_last_error",
@@ -56,6 +57,7 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_execute_host.argtypes = [vp, vp, vp, ci, vp]
     lib.dedisp_execute_host_async.argtypes = [vp, vp, vp, ci]
     lib.dedisp_host_sync.argtypes = [vp]
+    lib.dedisp_stream_block_async.argtypes = [vp, vp, i64, vp, i64, i64]
     lib.dedisp_plan_destroy.argtypes = [vp]
     lib.dedisp_variant_count.argtypes = []
     lib.dedisp_variant_name.argtypes = [ci]
@@ -177,6 +179,12 @@ class Plan:
         """Enqueue H2D + kernels + D2H on the plan's three-stream pipeline; see host_sync()."""
         _check(self._lib.dedisp_execute_host_async(self._h, _addr(h_in), _addr(h_out), int(nr_beams)),
                "dedisp_execute_host_async")
+
+    def stream_block_async(self, h_series, series_pitch: int, h_out, out_pitch: int, t0: int):
+        """One block of a long single-beam time series (see include/dedisp.h)."""
+        _check(self._lib.dedisp_stream_block_async(self._h, _addr(h_series), int(series_pitch),
+                                                   _addr(h_out), int(out_pitch), int(t0)),
+               "dedisp_stream_block_async")
 
     def host_sync(self):
         _check(self._lib.dedisp_host_sync(self._h), "dedisp_host_sync")

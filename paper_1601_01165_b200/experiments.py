@@ -1,6 +1,6 @@
-"""The paper's experiments on the current GPU (SURVEY.md 8(f) rows 1-3), as markdown tables.
+"""The paper's experiments on the current GPU (SURVEY.md 8(f) rows 1-4), as markdown tables.
 
-  python -m paper_1601_01165_b200.experiments [sweep] [zerodm] [histogram]
+  python -m paper_1601_01165_b200.experiments [sweep] [zerodm] [histogram] [stream]
 
 sweep     PAPER.md:105-107, Figs. 1-2: the two Table 2 setups (Apertif 1024 ch / 20 kHz / 1420 MHz / 300 MHz,
           LOFAR 32 ch / 200 kHz / 138 MHz / 6 MHz), trial DMs from 0 in steps of 0.25, 12 instances from 2 to
@@ -8,6 +8,8 @@ sweep     PAPER.md:105-107, Figs. 1-2: the two Table 2 setups (Apertif 1024 ch /
           and the speed-up over the no-reuse "generically tuned" kernel (Fig. 4).
 zerodm    PAPER.md:157-169 (section 4.3): all trial DMs equal to 0, i.e. perfect data reuse.
 histogram PAPER.md:151, Fig. 3: the distribution of GFLOP/s over the whole tuning space (every compiled variant).
+stream    the real-time setting: a long single-beam series in pinned host memory, dedispersed
+          in consecutive 1-s blocks with dedisp_stream_block_async (upload, kernels, download overlapped).
 
 Inputs are zeros of the right shape (values do not affect timing); parity is the tests' business.
 """
@@ -88,7 +90,38 @@ def histogram():
             print("  %7.0f - %7.0f GFLOP/s | %s %d" % (lo, hi, "#" * int(n), n))
 
 
+def stream(nblocks: int = 12):
+    import time
+
+    import torch
+
+    from . import tuning
+    print("| setup | blocks | ms per 1-s block, end to end | seconds of data per second | host<->device GB/s |")
+    print("|---|---|---|---|---|")
+    for s in (wl.APERTIF, wl.SURVEY8):
+        plan = dedisp.Plan(*s.plan_args())
+        tuning.apply_shipped(plan)
+        S, M = s.nr_samples, plan.max_shift
+        total = nblocks * S
+        in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
+        h_series = torch.zeros((s.nr_channels, total + M), dtype=in_dt).pin_memory()
+        h_out = torch.empty((s.nr_dms, total), dtype=torch.float32).pin_memory()
+        for b in range(3):   # warm-up: workspaces, kernel attributes
+            plan.stream_block_async(h_series, total + M, h_out, total, b * S)
+        plan.host_sync()
+        t0 = time.perf_counter()
+        for b in range(nblocks):
+            plan.stream_block_async(h_series, total + M, h_out, total, b * S)
+        plan.host_sync()
+        dt = (time.perf_counter() - t0) / nblocks
+        nbytes = s.nr_channels * (S + M) * h_series.element_size() + s.nr_dms * S * 4
+        print("| %s | %d | %.2f | %.0f | %.1f |" % (s.name, nblocks, dt * 1e3, s.seconds_of_data / dt,
+                                                    nbytes / dt / 1e9), flush=True)
+        plan.destroy()
+        del h_series, h_out
+
+
 if __name__ == "__main__":
-    what = sys.argv[1:] or ["sweep", "zerodm", "histogram"]
+    what = sys.argv[1:] or ["sweep", "zerodm", "histogram", "stream"]
     for w in what:
-        {"sweep": sweep, "zerodm": zerodm, "histogram": histogram}[w]()
+        {"sweep": sweep, "zerodm": zerodm, "histogram": histogram, "stream": stream}[w]()

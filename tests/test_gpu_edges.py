@@ -113,6 +113,38 @@ def test_execute_host_async_pipeline_matches_oracle(dd):
     plan.destroy()
 
 
+@pytest.mark.parametrize("u8", [False, True])
+def test_streaming_blocks_equal_one_long_dedispersion(dd, u8):
+    """dedisp_stream_block_async over 6 consecutive blocks of a long series (the blocks share M input
+    samples) equals the oracle run once on the whole series, bit-exactly."""
+    import torch
+    S, nblk = 1500, 6
+    s = wl.scaled(wl.SURVEY8 if u8 else wl.APERTIF, name="stream", nr_channels=48,
+                  channel_bw_MHz=300.0 / 48, nr_dms=61, nr_samples=S,
+                  values="u8" if u8 else "int16", in_dtype=wl.U8 if u8 else wl.F32)
+    plan = dd.Plan(*s.plan_args())
+    table = oracle.shift_table(*s.table_args())
+    M = plan.max_shift
+    total = nblk * S
+    long_setup = wl.scaled(s, nr_samples=total)
+    series = wl.make_input(long_setup, total + M, total + M + 5)[0]   # [C][pitch], odd pitch
+    ref = oracle.dedisperse(series[None], table, total)[0]
+    h_series = torch.from_numpy(series).pin_memory()
+    h_out = torch.full((s.nr_dms, total + 3), -1, dtype=torch.int32 if u8 else torch.float32).pin_memory()
+    for b in range(nblk):
+        plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, b * S)
+    plan.host_sync()
+    got = h_out.numpy()[:, :total]
+    if u8:
+        assert np.array_equal(got.view(np.uint32).astype(np.uint64), ref)
+    else:
+        assert np.array_equal(got.astype(np.float64), ref)
+    assert (h_out.numpy()[:, total:] == -1).all()     # nothing written past the blocks
+    with pytest.raises(dd.DedispError):
+        plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, total)  # past the end
+    plan.destroy()
+
+
 def test_argument_errors_on_device(dd):
     import torch
     s = wl.TINY
