@@ -62,11 +62,13 @@ def emit(dt: int, tt: int, qmax: int) -> str:
     # mask keeps the dispatch compare-and-branch (a chain of q == k tests with five or more cases is
     # turned into an indirect jump through a constant-memory table, LDC + BRX).
     o.append("    // rows: the thread's position in channel 0's staged row; ds: the warp's descriptor of")
-    o.append("    // channel 0 (stride wd words per channel), fetched one channel ahead of their use")
+    o.append("    // channel 0, WD words per channel; the descriptor of the next channel is fetched one channel")
+    o.append("    // ahead (after the last channel this reads one row past the chunk: in bounds, never used)")
+    o.append("    template <int WD>")
     o.append("    static __device__ __forceinline__ void chunk(float (&acc)[%d][%d], const float *rows, "
-             "const uint32_t *ds, int ncc, int lrow, int wd) {" % (dt, tt))
+             "const uint32_t *ds, int ncc, int lrow) {" % (dt, tt))
+    o.append("        const uint32_t *const ds_end = ds + ncc * WD;")
     o.append("        uint32_t d = tree_desc(ds), dn;")
-    o.append("        int cc = 0;")
     o.append("    NEXT:")
     for q in range(qmax):
         o.append("        if (d & %du) goto L%d;" % (0x100 << q, q))
@@ -74,14 +76,13 @@ def emit(dt: int, tt: int, qmax: int) -> str:
     for q in range(qmax + 1):
         o.append("    L%d:" % q)
         o.append("        do {")
-        o.append("            dn = d;")
-        o.append("            if (cc + 1 < ncc) dn = tree_desc(ds + (cc + 1) * wd);")
+        o.append("            ds += WD;")
+        o.append("            dn = tree_desc(ds);")
         o.append("            run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q)
         o.append("            rows += lrow;")
         o.append("            d = dn;")
-        o.append("            ++cc;")
-        o.append("        } while (cc < ncc && (d & %du));" % (0x100 << q))
-        o.append("        if (cc < ncc) goto NEXT;")
+        o.append("        } while (ds != ds_end && (d & %du));" % (0x100 << q))
+        o.append("        if (ds != ds_end) goto NEXT;")
         o.append("        goto END;")
     o.append("    END:;")
     o.append("    }")

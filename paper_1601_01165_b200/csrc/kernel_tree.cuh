@@ -57,7 +57,7 @@ __host__ __device__ inline size_t tree_fbuf_bytes(int lrow) {
 template <typename T>
 __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
     return T::NSTAGE * tree_stage_bytes<T>(lrow) + (T::U8 ? 3 * tree_fbuf_bytes<T>(lrow) : 0) +
-           (2 * T::NSTAGE + 3) * sizeof(uint64_t) + 16;
+           (2 * T::NSTAGE + 3) * sizeof(uint64_t) + 16 + T::WD * 4;
 }
 
 // Issue the copies of chunk k into its stage (called by one whole warp; lane l < CC stages channel
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             rows = reinterpret_cast<const float *>(st) + tw + lane * T::TT;
             ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
         }
-        TreeStep<T::DT, T::TT, T::QMAX>::chunk(acc, rows, ds, ncc, a.lrow, T::WD);
+        TreeStep<T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, rows, ds, ncc, a.lrow);
         if constexpr (!T::U8) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);

@@ -66,6 +66,7 @@ def test_lattice_walk_visits_the_right_offsets(dt, tt, qmax):
 def test_chunk_loop_dispatches_one_hot_slope_classes():
     text = gen_tree.emit(4, 28, 3)
     chunk = text.split("void chunk(")[1]
+    assert "dn = tree_desc(ds);" in chunk and "ds != ds_end" in chunk
     for q in range(3):
         assert "if (d & %du) goto L%d;" % (0x100 << q, q) in chunk
         assert "run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q in chunk
