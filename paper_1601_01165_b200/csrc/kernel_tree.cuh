@@ -151,16 +151,25 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
         const int ncc = (a.C - k * T::CC) < T::CC ? (a.C - k * T::CC) : T::CC;
         unsigned char *fb = stages + T::NSTAGE * sbytes + (size_t)(k % 3) * tree_fbuf_bytes<T>(a.lrow);
         float4 *frow = reinterpret_cast<float4 *>(fb);
-        const uint32_t *raw = reinterpret_cast<const uint32_t *>(st);
-        const int nwords = ncc * a.lrow / 4;  // 4 samples per 32-bit word
-        for (int i = threadIdx.x; i < nwords; i += T::THREADS) {
-            const uint32_t x = raw[i];
-            float4 v;  // byte b -> float: 0x4B000000 | b is 2^23 + b
-            v.x = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7650)) - 8388608.f;
-            v.y = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7651)) - 8388608.f;
-            v.z = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7652)) - 8388608.f;
-            v.w = __uint_as_float(__byte_perm(x, 0x4B000000u, 0x7653)) - 8388608.f;
-            frow[i] = v;
+        const uint4 *raw = reinterpret_cast<const uint4 *>(st);
+        const int n16 = ncc * a.lrow / 16;  // 16 samples per 128-bit load (lrow is a multiple of 16)
+        for (int i = threadIdx.x; i < n16; i += T::THREADS) {
+            const uint4 x = raw[i];
+            const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                // byte b -> float: 0x4B000000 | b is 2^23 + b; subtract 2^23 (two at a time)
+                float4 v;
+                v.x = __uint_as_float(__byte_perm(xs[m], 0x4B000000u, 0x7650));
+                v.y = __uint_as_float(__byte_perm(xs[m], 0x4B000000u, 0x7651));
+                v.z = __uint_as_float(__byte_perm(xs[m], 0x4B000000u, 0x7652));
+                v.w = __uint_as_float(__byte_perm(xs[m], 0x4B000000u, 0x7653));
+                asm("{.reg .b64 a, b; mov.b64 a, {%0, %1}; mov.b64 b, {%2, %2}; add.f32x2 a, a, b; "
+                    "mov.b64 {%0, %1}, a;}" : "+f"(v.x), "+f"(v.y) : "f"(-8388608.f));
+                asm("{.reg .b64 a, b; mov.b64 a, {%0, %1}; mov.b64 b, {%2, %2}; add.f32x2 a, a, b; "
+                    "mov.b64 {%0, %1}, a;}" : "+f"(v.z), "+f"(v.w) : "f"(-8388608.f));
+                frow[4 * i + m] = v;
+            }
         }
         uint32_t *fds = reinterpret_cast<uint32_t *>(fb + (size_t)T::CC * a.lrow * 4);
         if ((int)threadIdx.x < ncc * T::WD)
