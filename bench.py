@@ -36,8 +36,8 @@ FALLBACK_SM_MHZ = 1965.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the
 # same command (profiles/README.md says which file); None until captured for that config.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_tree_apertif.md: 116.9 MB read + 124.0 MB written per launch
-    "apertif": 116853248 + 124032512,
+    # profiles/r01_ncu_tree_apertif.md: 113.5 MB read + 122.2 MB written per launch
+    "apertif": 113459200 + 122203904,
 }
 
 
