@@ -38,6 +38,7 @@ struct VariantFit {
     bool ok = false;     // can run this plan
     int lrow = 0;        // shared-memory row pitch (elements)
     size_t smem = 0;     // dynamic shared memory bytes
+    int span = 0;        // largest shift difference across one of the variant's DM tiles
 };
 
 struct PlanShape {

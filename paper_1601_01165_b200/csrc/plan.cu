@@ -100,6 +100,7 @@ static void compute_fits(dedisp_plan *pl) {
             span = it->second;
         }
         pl->fit[v] = vs[v].fit(vs[v], p, span);
+        pl->fit[v].span = span;
     }
 }
 
@@ -147,23 +148,44 @@ static cudaError_t build_tree_tables(dedisp_plan *pl) {
     return e;
 }
 
-// Untuned default: a rough cost model (adds / kind rate, tile padding, wave quantisation).
+// Untuned default: a cost model in SM clocks.  A CTA costs the larger of its adds at the kind's
+// measured rate (adds/clk/SM on B200: tree ~58 for large thread tiles, lds ~28 = the one-word-per-add
+// shared-memory cap, generic ~10 = 4-byte loads at the L2's per-SM share) and of the bytes it stages
+// from L2 (~40 B/clk/SM); an SM runs ceil(CTAs / 148) of them (wave quantisation), more slowly when
+// too few warps are resident to hide latencies.  dedisp_tune replaces the guess by a measurement.
 static int heuristic_variant(const dedisp_plan *pl) {
     const auto &vs = variants();
     double best = 1e300;
     int bi = pl->dtype == DEDISP_U8 ? 1 : 0;
+    const double esz = pl->dtype == DEDISP_U8 ? 1 : 4;
     for (size_t v = 0; v < vs.size(); ++v) {
         if (!pl->fit[v].ok) continue;
         const Variant &x = vs[v];
-        double rate = x.kind == KIND_TREE ? 2.0 : x.kind == KIND_LDS ? 1.0 : 0.25;
-        double nd = std::ceil((double)pl->D / x.dms_cta), nt = std::ceil((double)pl->S / x.samples_cta);
-        double work = nd * x.dms_cta * nt * x.samples_cta;  // padded outputs
-        double ctas = nd * nt;
-        double occ = x.kind == KIND_GENERIC ? 8 : std::max(1.0, std::floor(227.0 * 1024 / (double)std::max<size_t>(pl->fit[v].smem, 1)));
-        occ = std::min(occ, std::floor(2048.0 / x.threads));
-        double slots = 148 * occ;
-        double waves = std::ceil(ctas / slots) / (ctas / slots);
-        double cost = work / rate * waves;
+        const double tile = (double)x.dt * x.tt;
+        double rate, need, occ;
+        if (x.kind == KIND_TREE) {
+            rate = (tile >= 100 ? (x.threads >= 384 ? 62 : 58) : tile >= 72 ? 52 : 42) *
+                   (pl->dtype == DEDISP_U8 ? 0.85 : 1.0);
+            need = 8;
+            occ = x.threads <= 128 ? 4 : (x.threads <= 256 && tile <= 48) ? 2 : 1;
+        } else if (x.kind == KIND_LDS) {
+            rate = tile >= 32 ? 28 : tile >= 16 ? 24 : 14;
+            need = 16;
+            occ = std::floor(227.0 * 1024 / (double)std::max<size_t>(pl->fit[v].smem, 1));
+            occ = std::max(1.0, std::min(occ, std::floor(2048.0 / x.threads)));
+        } else {
+            rate = 10;
+            need = 32;
+            occ = 8;
+        }
+        const double nd = std::ceil((double)pl->D / x.dms_cta), nt = std::ceil((double)pl->S / x.samples_cta);
+        const double adds_cta = (double)x.dms_cta * x.samples_cta * pl->C;
+        const double bytes_cta = x.kind == KIND_GENERIC ? 0 : (double)pl->C * (x.samples_cta + pl->fit[v].span) * esz;
+        const double t_cta = std::max(adds_cta / rate, bytes_cta / 40.0);
+        const double n_sm = std::ceil(nd * nt / 148.0);
+        const double resident = std::min(occ, n_sm);
+        const double warp_eff = std::min(1.0, resident * x.threads / 32.0 / need);
+        const double cost = n_sm * t_cta / warp_eff + 6000;  // + launch
         if (cost < best) { best = cost; bi = (int)v; }
     }
     return bi;
