@@ -36,8 +36,8 @@ FALLBACK_SM_MHZ = 1965.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the
 # same command (profiles/README.md says which file); None until captured for that config.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_tree_apertif.md: 113.5 MB read + 122.2 MB written per launch
-    "apertif": 113459200 + 122203904,
+    # profiles/r01_ncu_tree_apertif.md: 114.9 MB read + 123.9 MB written per launch
+    "apertif": 114913536 + 123922432,
 }
 
 

@@ -93,7 +93,10 @@ static Variant make_tree() {
     X(22, uint8_t, 12, 1, 4, 20, 8, 4, 4, 1) /* 48 x 640, 12 warps */      \
     X(23, uint8_t, 12, 1, 4, 28, 8, 4, 3, 1) /* 48 x 896, 12 warps, q <= 3 */ \
     X(24, uint8_t, 8, 1, 8, 20, 8, 4, 3, 1)  /* 64 x 640, q <= 3 */        \
-    X(25, uint8_t, 16, 1, 4, 12, 8, 4, 4, 1) /* 64 x 384, 16 warps */
+    X(25, uint8_t, 16, 1, 4, 12, 8, 4, 4, 1) /* 64 x 384, 16 warps */      \
+    X(26, float, 12, 1, 4, 28, 16, 3, 3, 1) /* 48 x 896, 12 warps, cc16 s3 */ \
+    X(27, float, 8, 1, 6, 28, 16, 3, 3, 1)  /* 48 x 896, cc16 s3 */        \
+    X(28, float, 12, 1, 4, 28, 12, 4, 3, 1) /* 48 x 896, 12 warps, cc12 s4 */
 
 #ifndef TREE_PART
 #define TREE_PART 0
