@@ -49,11 +49,14 @@ void register_tree25(std::vector<Variant> &);
 void register_tree26(std::vector<Variant> &);
 void register_tree27(std::vector<Variant> &);
 void register_tree28(std::vector<Variant> &);
+void register_tree29(std::vector<Variant> &);
+void register_tree30(std::vector<Variant> &);
+void register_tree31(std::vector<Variant> &);
 void register_tree(std::vector<Variant> &r) {
     void (*parts[])(std::vector<Variant> &) = {
         register_tree0, register_tree1, register_tree2, register_tree3, register_tree4, register_tree5, register_tree6, register_tree7, register_tree8, register_tree9, register_tree10, register_tree11, register_tree12, register_tree13, register_tree14, register_tree15, register_tree16, register_tree17, register_tree18, register_tree19,
         register_tree20, register_tree21, register_tree22, register_tree23, register_tree24,
-        register_tree25, register_tree26, register_tree27, register_tree28};
+        register_tree25, register_tree26, register_tree27, register_tree28, register_tree29, register_tree30, register_tree31};
     for (auto f : parts) f(r);
 }
 

@@ -96,7 +96,10 @@ static Variant make_tree() {
     X(25, uint8_t, 16, 1, 4, 12, 8, 4, 4, 1) /* 64 x 384, 16 warps */      \
     X(26, float, 12, 1, 4, 28, 16, 3, 3, 1) /* 48 x 896, 12 warps, cc16 s3 */ \
     X(27, float, 8, 1, 6, 28, 16, 3, 3, 1)  /* 48 x 896, cc16 s3 */        \
-    X(28, float, 12, 1, 4, 28, 12, 4, 3, 1) /* 48 x 896, 12 warps, cc12 s4 */
+    X(28, float, 12, 1, 4, 28, 12, 4, 3, 1) /* 48 x 896, 12 warps, cc12 s4 */ \
+    X(29, float, 12, 1, 5, 20, 16, 3, 3, 1) /* 60 x 640, 12 warps, cc16 s3 */ \
+    X(30, float, 12, 1, 4, 20, 16, 3, 4, 1) /* 48 x 640, 12 warps, cc16 s3, q <= 4 */ \
+    X(31, float, 16, 1, 6, 12, 16, 3, 4, 1) /* 96 x 384, 16 warps, cc16 s3, q <= 4 */
 
 #ifndef TREE_PART
 #define TREE_PART 0
