@@ -92,3 +92,33 @@ def test_shipped_winner_for_apertif_is_a_tree_kernel(dd):
     with dd.Plan(*wl.APERTIF.plan_args()) as plan:
         tuning.apply_shipped(plan)
         assert dd.variant_name(plan.variant).startswith("tree_f32")
+
+
+@pytest.mark.parametrize("name,kind", [("apertif", "tree_f32"), ("survey8", "tree_u8"),
+                                       ("lofar", "lds_f32"), ("batch40", "tree_f32")])
+def test_untuned_default_picks_the_right_kernel_family(dd, name, kind):
+    """Without a tuning cache the plan's cost model must land in the family the tuner picks
+    (DESIGN.md section 8)."""
+    with dd.Plan(*wl.CONFIGS[name].plan_args()) as plan:
+        assert dd.variant_name(plan.variant).startswith(kind)
+        assert plan.variant_supported(plan.variant)
+
+
+def test_long_shift_setup_uses_a_staged_kernel(dd):
+    """The paper's LOFAR setup (DM step 0.25: hundreds of samples per DM step): tree kernels are out,
+    the long-span lds variants fit; every supported variant stays exact."""
+    s = wl.Setup("lofar_paper_s", 32, 138.0, 6.0 / 32, 200000.0, 9000, 0.0, 0.25, 24, values="int16",
+                 seed=77)
+    plan, table, x, d_in = make_case(dd, s)
+    assert not tree_variants(dd, plan)
+    names = [dd.variant_name(v) for v in plan.supported_variants()]
+    assert any(n.startswith("lds_f32: 4x2048") or n.startswith("lds_f32: 4x4096") for n in names)
+    ref = oracle.dedisperse(x, table, s.nr_samples)
+    ran = 0
+    for v in plan.supported_variants():
+        d_out = out_buffer(s, fill=-1.0)
+        plan.execute_variant(v, d_in, d_out)
+        assert np.array_equal(to_host(s, d_out).astype(np.float64), ref), dd.variant_name(v)
+        ran += 1
+    assert ran >= 3
+    plan.destroy()
