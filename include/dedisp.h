@@ -55,7 +55,8 @@ enum {
     DEDISP_NR_DMS = 6,
     DEDISP_NR_SAMPLES = 7,
     DEDISP_IN_DTYPE = 8,
-    DEDISP_MAX_STEP = 9    /* max over (c, i) of shift(c, i+1) - shift(c, i) */
+    DEDISP_MAX_STEP = 9,   /* max over (c, i) of shift(c, i+1) - shift(c, i) */
+    DEDISP_RESERVED_BEAMS = 10 /* U8 plans: beams the pair workspace holds (dedisp_plan_reserve); else 0 */
 };
 
 /*
@@ -66,10 +67,14 @@ enum {
  *     x    = ((4150*dm_i) * (1/(f_c*f_c) - 1/(f_h*f_h))) * sample_rate          (Eq. 1)
  *     shift(c,i) = floor(x) + (x - floor(x) >= 0.5)
  * Chooses the kernel variant (tuning cache named by $DEDISP_TUNE_CACHE if set, else a
- * heuristic).  nr_samples = S, output samples per beam.
+ * heuristic) and prepares it (function attributes, its descriptor table).  nr_samples = S,
+ * output samples per beam.  The plan belongs to the CUDA device that is current at creation;
+ * every later call on it must be made with the same device current.  U8 plans also allocate
+ * the pair workspace for one beam (dedisp_plan_reserve).
  * Errors: INVALID_ARG (plan == NULL, C/D/S < 1, f_low/bw/rate <= 0 or non-finite,
- * dm_first/dm_step < 0 or non-finite, unknown dtype); OVERFLOW (shift or S+M > INT32_MAX,
- * or C*255 >= 2^32 for U8); ALLOC; CUDA.  On error *plan = NULL.
+ * dm_first/dm_step < 0 or non-finite, unknown dtype, or no compiled kernel variant can run the
+ * plan); OVERFLOW (shift or S+M > INT32_MAX, or C*255 >= 2^32 for U8); ALLOC; CUDA.  On error
+ * *plan = NULL.
  */
 int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
                        double channel_bw_MHz, double sample_rate, int64_t nr_samples,
@@ -82,6 +87,17 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
  * Errors: INVALID_ARG (null), CUDA, ALLOC.
  */
 int dedisp_shift_table(const dedisp_plan *plan, int32_t *host_out);
+
+/*
+ * dedisp_plan_reserve -- U8 plans only (a no-op returning OK for F32 plans): the uint8 register-window
+ * kernels read the input through a plan-owned device workspace holding every input row as pairs of
+ * samples about S/2 apart (two 16-bit counters per 32-bit add; 4 bytes per pair, C * (S/2 + M) pairs
+ * per beam).  dedisp_plan_create allocates it for one beam; this call grows it to nr_beams beams so
+ * that dedisp_execute runs a whole batch in one kernel launch.  Without it a larger batch still
+ * works: dedisp_execute then goes through the workspace as many beams at a time as it holds.
+ * Synchronises the device and allocates; never shrinks.  Errors: INVALID_ARG, ALLOC, CUDA.
+ */
+int dedisp_plan_reserve(dedisp_plan *plan, int nr_beams);
 
 /* dedisp_plan_get -- scalar queries (see the enum).  Errors: INVALID_ARG. */
 int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value);
@@ -96,17 +112,23 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value);
  *          borrowed, fully overwritten, base 16-byte aligned.
  *   stream: a cudaStream_t (NULL = default stream).
  * Asynchronous: enqueues kernels on `stream` and returns; no host sync, no allocation,
- * no host<->device copy.  fp32 sums are accumulated in fp32 in ascending channel order.
- * The same plan may be executed repeatedly and concurrently on different streams.
- * Errors: INVALID_ARG (null, nr_beams < 1, misaligned base), CUDA (launch error).
+ * no host<->device copy, no function-attribute call (all of that happened when the variant
+ * was selected), so the first call on a fresh plan can already be captured into a CUDA graph.
+ * fp32 sums are accumulated in fp32 in ascending channel order.
+ * An F32 plan may be executed repeatedly and concurrently on different streams.  A U8 plan may
+ * be executed repeatedly, but calls on ONE U8 plan must be ordered with respect to each other
+ * (same stream, or events): they share the plan's pair workspace (dedisp_plan_reserve).
+ * Errors: INVALID_ARG (null, nr_beams < 1, misaligned base, current device is not the plan's),
+ * CUDA (launch error).
  */
 int dedisp_execute(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
                    void *stream);
 
 /*
- * dedisp_execute_variant -- dedisp_execute with an explicit kernel variant (same contract; used by
- * the tuner and the parity tests to drive every compiled variant).  INVALID_ARG if the variant
- * does not support the plan.
+ * dedisp_execute_variant -- dedisp_execute with an explicit kernel variant (used by the tuner and the
+ * parity tests to drive every compiled variant).  Same contract, except that the first use of a
+ * variant on a plan prepares it (one cudaFuncSetAttribute, and for tree variants one descriptor-table
+ * allocation and build).  INVALID_ARG if the variant does not support the plan.
  */
 int dedisp_execute_variant(const dedisp_plan *plan, int variant, const void *d_in, void *d_out,
                            int nr_beams, void *stream);
@@ -171,7 +193,8 @@ const char *dedisp_variant_name(int variant);
 /* 1 if `variant` can run this plan (dtype, alignment, shared-memory fit), else 0. */
 int dedisp_variant_supported(const dedisp_plan *plan, int variant);
 
-/* Select the variant execute() launches.  Errors: INVALID_ARG if unsupported. */
+/* Select the variant execute() launches and prepare it (function attribute, descriptor table).
+ * Errors: INVALID_ARG if unsupported, ALLOC, CUDA. */
 int dedisp_plan_set_variant(dedisp_plan *plan, int variant);
 
 /*
@@ -179,16 +202,19 @@ int dedisp_plan_set_variant(dedisp_plan *plan, int variant);
  * combinations and select the best performing one"): times every supported variant on the
  * caller's buffers (same contract as dedisp_execute; d_out is overwritten) with CUDA events
  * on `stream` (synchronises), selects the fastest, and, if cache_path != NULL, persists
- * the winner (one text line "key<TAB>variant name<TAB>note" keyed by GPU name + setup, appended;
- * the last matching line wins on load).  ms_out (host, may be NULL)
+ * the winner (one text line "key<TAB>variant name<TAB>note", appended; the last matching line
+ * wins on load).  The key is GPU name + setup + a batch-size class (1 beam / 2-7 / 8 or more:
+ * the best tile differs when one beam leaves the last wave of CTAs part empty).  ms_out (host, may be NULL)
  * receives variant_count floats: mean ms per call, or -1 for unsupported variants.
  */
 int dedisp_tune(dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams, void *stream,
                 const char *cache_path, float *ms_out);
 
-/* Load a winner persisted by dedisp_tune.  Returns OK and leaves the plan unchanged if the
- * file has no entry for this setup; IO if the file cannot be opened. */
-int dedisp_plan_load_tuning(dedisp_plan *plan, const char *cache_path);
+/* Load a winner persisted by dedisp_tune for batches of nr_beams beams (the batch-size class of
+ * the key; an entry of another class is used if the file has none for this one).  Returns OK and
+ * leaves the plan unchanged if the file has no entry for this setup; IO if the file cannot be
+ * opened.  *hit (may be NULL) is set to 1 if an entry was applied, else 0. */
+int dedisp_plan_load_tuning(dedisp_plan *plan, const char *cache_path, int nr_beams, int *hit);
 
 const char *dedisp_status_string(int status);
 

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -28,9 +29,13 @@ struct KArgs {
     int S;                   // output samples per beam
     int in_pitch;            // elements per input row (multiple of 16 bytes)
     int dpitch;              // ints per shiftT row (multiple of 128, >= D + 128)
-    int lrow;                // shared-memory row pitch in elements (tiled kernels)
+    int lrow;                // shared-memory row pitch in staged elements (tiled kernels)
+    const uint32_t *pairs;   // uint8 tree kernels: [B][C][pair_pitch] 16-bit sample pairs (workspace)
+    int pair_pitch;          // pairs per row (multiple of 4)
+    int S2;                  // pair y holds samples y and y + S2 (about S/2, multiple of 4)
     const uint32_t *desc;    // KIND_TREE: [C][descpitch] descriptors for the variant's tile
     int descpitch;
+    uint32_t zero, one;      // 0 and 1 the compiler cannot see (uint8 tree kernels, gen_tree.py)
 };
 
 // Per-variant numbers derived from the plan's shift table at plan creation.
@@ -43,6 +48,7 @@ struct VariantFit {
 
 struct PlanShape {
     int C, D, S, in_pitch, dtype;
+    int S2;                  // uint8 pair layout: distance of the two samples of a pair
     int64_t M;               // max shift
     int max_step;            // max over (c,i) of shift(c,i+1)-shift(c,i)
     const int32_t *h_shift;  // host copy [D][C]
@@ -55,11 +61,12 @@ struct TreeTable {
     int dt = 0, dms_cta = 0;
     uint32_t *d_desc = nullptr;  // [C][pitch]
     int pitch = 0;
-    bool valid = false;          // every woff fits 16 bits
 };
 struct TreeInfo {
     bool valid = false;  // every channel's increments are {q_c, q_c + 1}, q_c <= 7
     int qmax = -1;       // max_c q_c
+    int *d_qc = nullptr; // device: q_c per channel
+    std::mutex mu;       // guards tables (built when a tree variant is first selected or run)
     std::vector<TreeTable> tables;
     const TreeTable *find(int dt, int dms_cta) const {
         for (const TreeTable &t : tables)
@@ -77,7 +84,7 @@ struct Variant {
     int dt, tt;       // outputs per thread: dt DMs x tt samples
     int cc;           // channel-chunk depth (channels per pipeline stage)
     int stages;
-    int rstep;        // KIND_TREE: largest slope class q_c the variant's lattice covers (QMAX)
+    int qmax;         // KIND_TREE: largest slope class q_c the variant's lattice covers
     int threads;
     // Fills lrow/smem, returns whether the variant supports the plan.
     VariantFit (*fit)(const Variant &, const PlanShape &, int span_cta);
@@ -85,12 +92,8 @@ struct Variant {
     cudaError_t (*prepare)(size_t smem);  // cudaFuncSetAttribute for large dynamic smem
 };
 
+// The registry: one entry per line of csrc/variants.py, in that order (build/registry_gen.inc).
 const std::vector<Variant> &variants();
-// Each variants_*.cu appends its instantiations.
-void register_generic(std::vector<Variant> &);
-void register_lds(std::vector<Variant> &);
-void register_u8(std::vector<Variant> &);
-void register_tree(std::vector<Variant> &);
 
 // shift_table.cu
 cudaError_t build_shift_tables(int C, double f_low, double bw, double rate, double dm_first,
@@ -102,6 +105,9 @@ cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch,
 cudaError_t build_tree_desc(const int32_t *d_shiftT, const int *d_qc, int C, int D, int dpitch,
                             int dt, int dms_cta, int al, int descpitch, uint32_t *d_desc,
                             int *d_flags, cudaStream_t st);
+
+cudaError_t pack_pairs(const uint8_t *d_in, uint32_t *d_pairs, int nr_beams, int C, int in_pitch,
+                       int pair_pitch, int S2, cudaStream_t st);
 
 void set_last_error(const char *what, cudaError_t e);
 
@@ -131,6 +137,11 @@ struct dedisp_plan {
     std::vector<dedisp::VariantFit> fit;  // per variant
     dedisp::TreeInfo tree;
     int variant = 0;
+    int device = 0;                // the CUDA device the plan's tables live on
+    // uint8 tree kernels: the input repacked as pairs of samples S2 apart (pack_pairs_kernel)
+    int S2 = 0, pair_pitch = 0;
+    uint32_t *d_pairs = nullptr;   // [pairs_beams][C][pair_pitch]
+    int pairs_beams = 0;
     // host-buffer path workspace (dedisp_execute_host)
     void *ws_in = nullptr, *ws_out = nullptr;
     size_t ws_in_bytes = 0, ws_out_bytes = 0;

@@ -14,7 +14,11 @@ the bits b_j are warp-uniform, so the selection is a walk through nodes N[q][j][
 two-way branches: one test per DM, no indirect jump, no dynamic register index.  Per (DT, TT, QMAX)
 the generator emits one lattice function per q and the channel loop of a staged chunk around them.
 
-Usage: python gen_tree.py OUT.cuh DT,TT,QMAX [DT,TT,QMAX ...]
+Two element types: "f32" (fp32 input: float accumulators, FADD / packed FADD2) and "u32" (uint8 input
+staged as pairs of 16-bit counters in one 32-bit word, kernel_tree.cuh: one integer add does two adds
+whatever the offset).
+
+Usage: python gen_tree.py OUT.cuh TYPE:DT,TT,QMAX [TYPE:DT,TT,QMAX ...]
 """
 from __future__ import annotations
 
@@ -26,21 +30,28 @@ def wn(dt: int, tt: int, q: int) -> int:
     return (3 + (dt - 1) * (q + 1) + tt + 3) // 4 * 4
 
 
-def emit(dt: int, tt: int, qmax: int) -> str:
+CTYPE = {"f32": ("float", "float4"), "u32": ("uint32_t", "uint4")}
+
+
+def emit(dt: int, tt: int, qmax: int, typ: str = "f32") -> str:
     o = []
     wnmax = wn(dt, tt, qmax)
-    o.append("template <> struct TreeStep<%d, %d, %d> {" % (dt, tt, qmax))
+    ct, vt = CTYPE[typ]
+    # u32: two warp-uniform run-time constants (0 and 1) that pin the pipe of each add, see tree_add
+    xdecl = ", uint32_t zero, uint32_t one" if typ == "u32" else ""
+    xargs = ", zero, one" if typ == "u32" else ""
+    o.append("template <> struct TreeStep<%s, %d, %d, %d> {" % (ct, dt, tt, qmax))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
     # one lattice per slope class q
     for q in range(qmax + 1):
         n = wn(dt, tt, q)
         o.append("    // slope class q = %d.  p: 16-byte aligned window start in shared memory; m0, bits: "
                  "warp-uniform" % q)
-        o.append("    static __device__ __forceinline__ void run_q%d(float (&acc)[%d][%d], const float *p, "
-                 "unsigned m0, unsigned bits) {" % (q, dt, tt))
-        o.append("        float w[%d];" % n)
-        o.append("        float4 v;")
-        o.append("        const float4 *p4 = reinterpret_cast<const float4 *>(p);")
+        o.append("    static __device__ __forceinline__ void run_q%d(%s (&acc)[%d][%d], const %s *p, "
+                 "unsigned m0, unsigned bits%s) {" % (q, ct, dt, tt, ct, xdecl))
+        o.append("        %s w[%d];" % (ct, n))
+        o.append("        %s v;" % vt)
+        o.append("        const %s *p4 = reinterpret_cast<const %s *>(p);" % (vt, vt))
         for m in range(n // 4):
             o.append("        v = p4[%d]; w[%d] = v.x; w[%d] = v.y; w[%d] = v.z; w[%d] = v.w;"
                      % (m, 4 * m, 4 * m + 1, 4 * m + 2, 4 * m + 3))
@@ -49,7 +60,7 @@ def emit(dt: int, tt: int, qmax: int) -> str:
         for j in range(dt):
             for r in range(j * q, j * q + 3 + j + 1):
                 o.append("    N_%d_%d:" % (j, r))
-                o.append("        tree_add<%d, %d>(acc[%d], w);" % (r, tt, j))
+                o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
                 if j + 1 < dt:
                     o.append("        if (bits & %du) goto N_%d_%d; else goto N_%d_%d;"
                              % (1 << j, j + 1, r + q + 1, j + 1, r + q))
@@ -65,8 +76,8 @@ def emit(dt: int, tt: int, qmax: int) -> str:
     o.append("    // channel 0, WD words per channel; the descriptor of the next channel is fetched one channel")
     o.append("    // ahead (after the last channel this reads one row past the chunk: in bounds, never used)")
     o.append("    template <int WD>")
-    o.append("    static __device__ __forceinline__ void chunk(float (&acc)[%d][%d], const float *rows, "
-             "const uint32_t *ds, int ncc, int lrow) {" % (dt, tt))
+    o.append("    static __device__ __forceinline__ void chunk(%s (&acc)[%d][%d], const %s *rows, "
+             "const uint32_t *ds, int ncc, int lrow%s) {" % (ct, dt, tt, ct, xdecl))
     o.append("        const uint32_t *const ds_end = ds + ncc * WD;")
     o.append("        uint32_t d = tree_desc(ds), dn;")
     o.append("    NEXT:")
@@ -78,7 +89,7 @@ def emit(dt: int, tt: int, qmax: int) -> str:
         o.append("        do {")
         o.append("            ds += WD;")
         o.append("            dn = tree_desc(ds);")
-        o.append("            run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q)
+        o.append("            run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu%s);" % (q, xargs))
         o.append("            rows += lrow;")
         o.append("            d = dn;")
         o.append("        } while (ds != ds_end && (d & %du));" % (0x100 << q))
@@ -94,7 +105,7 @@ HEADER = """// GENERATED by gen_tree.py -- do not edit.  KIND_TREE add lattices 
 #pragma once
 #include <stdint.h>
 namespace dedisp {
-template <int DT, int TT, int QMAX> struct TreeStep;
+template <typename E, int DT, int TT, int QMAX> struct TreeStep;
 // descriptor of one (channel, DM group): a shared-memory load whose address is the same for the whole
 // warp.  Explicit ld.shared keeps it out of the generic address space, whose loads the compiler's
 // divergence analysis treats as divergent.
@@ -125,15 +136,34 @@ __device__ __forceinline__ void tree_add(float (&acc)[TT], const float (&w)[WN])
             asm volatile("add.f32 %0, %0, %1;" : "+f"(acc[k]) : "f"(w[R + k]));
     }
 }
+// uint8 input: acc and w hold two 16-bit counters / samples per word, so one 32-bit add does two adds
+// whatever the offset.  Integer adds issue at half rate on either of two pipes: IADD3 on the integer
+// pipe, IMAD on the FMA pipe.  Left to itself ptxas turns three of four adds into IMAD.IADD (84
+// lanes/clk/SM measured); alternating a three-input IADD3 (+ a run-time zero) with an IMAD (x a
+// run-time one), neither of which it can rewrite, reaches 115 (profiles/r02_microbench.md).
+template <int R, int TT, int WN>
+__device__ __forceinline__ void tree_add(uint32_t (&acc)[TT], const uint32_t (&w)[WN], uint32_t zero,
+                                         uint32_t one) {
+    static_assert(R + TT <= WN, "window too short");
+#pragma unroll
+    for (int k = 0; k < TT; ++k) {
+        if (k % 2 == 0)
+            asm volatile("{.reg .u32 t; add.u32 t, %1, %2; add.u32 %0, %0, t;}"
+                         : "+r"(acc[k]) : "r"(w[R + k]), "r"(zero));
+        else
+            asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc[k]) : "r"(w[R + k]), "r"(one));
+    }
+}
 """
 
 
 def main(argv):
     out = argv[1]
-    combos = sorted({tuple(int(x) for x in a.split(",")) for a in argv[2:]})
+    combos = sorted({(a.split(":")[0],) + tuple(int(x) for x in a.split(":")[1].split(","))
+                     for a in argv[2:]})
     parts = [HEADER]
-    for dt, tt, qmax in combos:
-        parts.append(emit(dt, tt, qmax))
+    for typ, dt, tt, qmax in combos:
+        parts.append(emit(dt, tt, qmax, typ))
     parts.append("}  // namespace dedisp\n")
     text = "\n".join(parts)
     try:

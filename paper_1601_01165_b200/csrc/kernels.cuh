@@ -86,14 +86,13 @@ __global__ void __launch_bounds__(256) generic_kernel(KArgs a) {
 // ---------------------------------------------------------------- tiled kernels
 // Compile-time tile description.
 //   WD x WT consumer warps: WD DM groups of DT DMs, WT time chunks of 32*TT samples.
-//   CC channels per pipeline stage, NSTAGE stages (RSTEP_ is unused, kept for the variant tables).
-template <typename In_, int KIND_, int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_,
-          int RSTEP_, int MINB_>
+//   CC channels per pipeline stage, NSTAGE stages.
+template <typename In_, int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_, int MINB_>
 struct Tile {
     typedef In_ In;
     typedef typename AccOf<In_>::type Acc;
-    static constexpr int KIND = KIND_, WD = WD_, WT = WT_, DT = DT_, TT = TT_, CC = CC_,
-                         NSTAGE = NSTAGE_, RSTEP = RSTEP_, MINB = MINB_;
+    static constexpr int WD = WD_, WT = WT_, DT = DT_, TT = TT_, CC = CC_, NSTAGE = NSTAGE_,
+                         MINB = MINB_;
     static constexpr int NW = WD * WT;              // consumer warps
     static constexpr int THREADS = (NW + 1) * 32;   // + producer warp
     static constexpr int DMS_CTA = WD * DT;
@@ -122,9 +121,28 @@ __device__ __forceinline__ void channel_lds(typename T::Acc (&acc)[T::DT][T::TT]
                                             const typename T::In *row, const int32_t *sh, int g,
                                             int tw, int lane) {
     const int base = sh[0] & ~(T::AL - 1);
+    // the group's DT shifts: warp-uniform (broadcast) loads, four at a time where DT allows -- each is
+    // a shared-memory wavefront, and wavefronts are what bounds this kernel
+    int s[T::DT];
+    if constexpr (T::DT % 4 == 0) {
+#pragma unroll
+        for (int j = 0; j < T::DT; j += 4) {
+            const int4 v = *reinterpret_cast<const int4 *>(sh + g * T::DT + j);
+            s[j] = v.x; s[j + 1] = v.y; s[j + 2] = v.z; s[j + 3] = v.w;
+        }
+    } else if constexpr (T::DT % 2 == 0) {
+#pragma unroll
+        for (int j = 0; j < T::DT; j += 2) {
+            const int2 v = *reinterpret_cast<const int2 *>(sh + g * T::DT + j);
+            s[j] = v.x; s[j + 1] = v.y;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < T::DT; ++j) s[j] = sh[g * T::DT + j];
+    }
 #pragma unroll
     for (int j = 0; j < T::DT; ++j) {
-        const typename T::In *p = row + (sh[g * T::DT + j] - base) + tw + lane;
+        const typename T::In *p = row + (s[j] - base) + tw + lane;
 #pragma unroll
         for (int k = 0; k < T::TT; ++k) acc[j][k] += (typename T::Acc)p[32 * k];
     }

@@ -19,55 +19,13 @@ void set_last_error(const char *what, cudaError_t e) {
     snprintf(g_last_error, sizeof g_last_error, "%s: %s", what, cudaGetErrorString(e));
 }
 
-// one per row of TREE_VARIANTS in variants_tree.cu
-void register_tree0(std::vector<Variant> &);
-void register_tree1(std::vector<Variant> &);
-void register_tree2(std::vector<Variant> &);
-void register_tree3(std::vector<Variant> &);
-void register_tree4(std::vector<Variant> &);
-void register_tree5(std::vector<Variant> &);
-void register_tree6(std::vector<Variant> &);
-void register_tree7(std::vector<Variant> &);
-void register_tree8(std::vector<Variant> &);
-void register_tree9(std::vector<Variant> &);
-void register_tree10(std::vector<Variant> &);
-void register_tree11(std::vector<Variant> &);
-void register_tree12(std::vector<Variant> &);
-void register_tree13(std::vector<Variant> &);
-void register_tree14(std::vector<Variant> &);
-void register_tree15(std::vector<Variant> &);
-void register_tree16(std::vector<Variant> &);
-void register_tree17(std::vector<Variant> &);
-void register_tree18(std::vector<Variant> &);
-void register_tree19(std::vector<Variant> &);
-void register_tree20(std::vector<Variant> &);
-void register_tree21(std::vector<Variant> &);
-void register_tree22(std::vector<Variant> &);
-void register_tree23(std::vector<Variant> &);
-void register_tree24(std::vector<Variant> &);
-void register_tree25(std::vector<Variant> &);
-void register_tree26(std::vector<Variant> &);
-void register_tree27(std::vector<Variant> &);
-void register_tree28(std::vector<Variant> &);
-void register_tree29(std::vector<Variant> &);
-void register_tree30(std::vector<Variant> &);
-void register_tree31(std::vector<Variant> &);
-void register_tree(std::vector<Variant> &r) {
-    void (*parts[])(std::vector<Variant> &) = {
-        register_tree0, register_tree1, register_tree2, register_tree3, register_tree4, register_tree5, register_tree6, register_tree7, register_tree8, register_tree9, register_tree10, register_tree11, register_tree12, register_tree13, register_tree14, register_tree15, register_tree16, register_tree17, register_tree18, register_tree19,
-        register_tree20, register_tree21, register_tree22, register_tree23, register_tree24,
-        register_tree25, register_tree26, register_tree27, register_tree28, register_tree29, register_tree30, register_tree31};
-    for (auto f : parts) f(r);
-}
+#include "build/registry_gen.inc"  // generated from variants.py: kVariantMakers[]
 
 const std::vector<Variant> &variants() {
     static std::vector<Variant> reg;
     static std::once_flag once;
     std::call_once(once, [] {
-        register_generic(reg);  // variants 0 (f32) and 1 (u8): the no-reuse baseline
-        register_lds(reg);
-        register_u8(reg);
-        register_tree(reg);
+        for (auto make : kVariantMakers) reg.push_back(make());
     });
     return reg;
 }
@@ -87,7 +45,7 @@ static int span_for(const PlanShape &p, int dms) {
 static PlanShape shape_of(const dedisp_plan *pl) {
     PlanShape p;
     p.C = pl->C; p.D = pl->D; p.S = (int)pl->S; p.in_pitch = pl->in_pitch; p.dtype = pl->dtype;
-    p.M = pl->M; p.max_step = pl->max_step; p.h_shift = pl->h_shift.data();
+    p.M = pl->M; p.max_step = pl->max_step; p.h_shift = pl->h_shift.data(); p.S2 = pl->S2;
     p.tree = &pl->tree;
     return p;
 }
@@ -110,48 +68,76 @@ static void compute_fits(dedisp_plan *pl) {
     }
 }
 
-// KIND_TREE tables: per-channel slope classes, then one descriptor table per (DT, DMs per CTA)
-// pair some registered variant uses.
-static cudaError_t build_tree_tables(dedisp_plan *pl) {
+// KIND_TREE tables, part 1 (plan creation): per-channel slope classes q_c, kept on the device for the
+// descriptor builds.
+static cudaError_t build_tree_slopes(dedisp_plan *pl) {
     if (pl->C > 65535) return cudaSuccess;  // grid.y of desc_kernel; such plans use other kinds
-    int *d_flags = nullptr, *d_qc = nullptr;
+    int *d_flags = nullptr;
     int h[2] = {0, 0};
     cudaError_t e;
-    if ((e = cudaMalloc(&d_flags, 8)) != cudaSuccess || (e = cudaMalloc(&d_qc, (size_t)pl->C * 4)) != cudaSuccess ||
+    if ((e = cudaMalloc(&d_flags, 8)) != cudaSuccess ||
+        (e = cudaMalloc(&pl->tree.d_qc, (size_t)pl->C * 4)) != cudaSuccess ||
         (e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
-        (e = build_chan_slopes(pl->d_shiftT, pl->C, pl->D, pl->dpitch, d_qc, d_flags, 0)) != cudaSuccess ||
-        (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess) {
+        (e = build_chan_slopes(pl->d_shiftT, pl->C, pl->D, pl->dpitch, pl->tree.d_qc, d_flags, 0)) != cudaSuccess ||
+        (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess)
         set_last_error("build_chan_slopes", e);
-        cudaFree(d_flags);
-        cudaFree(d_qc);
-        return e;
-    }
+    cudaFree(d_flags);
+    if (e != cudaSuccess) return e;
     pl->tree.qmax = h[0];
     pl->tree.valid = h[1] == 0;
-    if (pl->tree.valid) {
-        for (const Variant &v : variants()) {
-            if (v.kind != KIND_TREE || v.dtype != pl->dtype || v.rstep < pl->tree.qmax) continue;
-            if (pl->tree.find(v.dt, v.dms_cta)) continue;
-            TreeTable t;
-            t.dt = v.dt;
-            t.dms_cta = v.dms_cta;
-            const int nG = (pl->D + v.dt - 1) / v.dt;
-            t.pitch = (nG + 31) / 32 * 32 + 32;
-            if ((e = cudaMalloc(&t.d_desc, (size_t)pl->C * t.pitch * 4)) != cudaSuccess) break;
-            pl->tree.tables.push_back(t);  // owned by the plan from here on
-            if ((e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
-                (e = build_tree_desc(pl->d_shiftT, d_qc, pl->C, pl->D, pl->dpitch, v.dt, v.dms_cta,
-                                     pl->dtype == DEDISP_U8 ? 16 : 4, t.pitch, t.d_desc, d_flags,
-                                     0)) != cudaSuccess ||
-                (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess)
-                break;
-            pl->tree.tables.back().valid = h[1] == 0;
-        }
-        if (e != cudaSuccess) set_last_error("build_tree_desc", e);
+    return cudaSuccess;
+}
+
+// Part 2 (when a tree variant is selected or first run): the descriptor table of the variant's
+// (DT, DMs per CTA) pair.  Only the variants that run pay for a table (4 bytes per channel and DM
+// group); a failed allocation leaves the plan usable with every other variant.
+static int ensure_tree_table(dedisp_plan *pl, int v) {
+    const Variant &x = variants()[v];
+    if (x.kind != KIND_TREE) return DEDISP_OK;
+    std::lock_guard<std::mutex> lk(pl->tree.mu);
+    if (pl->tree.find(x.dt, x.dms_cta)) return DEDISP_OK;
+    TreeTable t;
+    t.dt = x.dt;
+    t.dms_cta = x.dms_cta;
+    const int nG = (pl->D + x.dt - 1) / x.dt;
+    t.pitch = (nG + 31) / 32 * 32 + 32;
+    int *d_flags = nullptr;
+    int h[2] = {0, 0};
+    cudaError_t e;
+    if ((e = cudaMalloc(&t.d_desc, (size_t)pl->C * t.pitch * 4)) != cudaSuccess) {
+        set_last_error("cudaMalloc(descriptors)", e);
+        return DEDISP_ERR_ALLOC;
+    }
+    if ((e = cudaMalloc(&d_flags, 8)) != cudaSuccess || (e = cudaMemset(d_flags, 0, 8)) != cudaSuccess ||
+        (e = build_tree_desc(pl->d_shiftT, pl->tree.d_qc, pl->C, pl->D, pl->dpitch, x.dt, x.dms_cta, 4,
+                             t.pitch, t.d_desc, d_flags, 0)) != cudaSuccess ||
+        (e = cudaMemcpy(h, d_flags, 8, cudaMemcpyDeviceToHost)) != cudaSuccess) {
+        set_last_error("build_tree_desc", e);
+        cudaFree(t.d_desc);
+        if (d_flags) cudaFree(d_flags);
+        return DEDISP_ERR_CUDA;
     }
     cudaFree(d_flags);
-    cudaFree(d_qc);
-    return e;
+    if (h[1] != 0) {  // a window offset past 16 bits: tree_fit excludes such plans
+        cudaFree(t.d_desc);
+        return DEDISP_ERR_INVALID_ARG;
+    }
+    pl->tree.tables.push_back(t);
+    return DEDISP_OK;
+}
+
+// Everything a variant needs before its first launch, done when it is SELECTED (plan creation,
+// set_variant, load_tuning, tune) so that dedisp_execute itself neither allocates nor touches
+// function attributes: the large-shared-memory attribute (per device: set unconditionally, it is
+// cheap) and, for tree variants, the descriptor table.
+static int prepare_variant(dedisp_plan *pl, int v) {
+    const VariantFit &f = pl->fit[v];
+    if (!f.ok) return DEDISP_ERR_INVALID_ARG;
+    if (f.smem > 48 * 1024) {
+        cudaError_t e = variants()[v].prepare(f.smem);
+        if (e != cudaSuccess) { set_last_error("cudaFuncSetAttribute", e); return DEDISP_ERR_CUDA; }
+    }
+    return ensure_tree_table(pl, v);
 }
 
 // Untuned default: a cost model in SM clocks.  A CTA costs the larger of its adds at the kind's
@@ -162,7 +148,7 @@ static cudaError_t build_tree_tables(dedisp_plan *pl) {
 static int heuristic_variant(const dedisp_plan *pl) {
     const auto &vs = variants();
     double best = 1e300;
-    int bi = pl->dtype == DEDISP_U8 ? 1 : 0;
+    int bi = -1;  // no variant supports the plan: dedisp_plan_create reports it
     const double esz = pl->dtype == DEDISP_U8 ? 1 : 4;
     for (size_t v = 0; v < vs.size(); ++v) {
         if (!pl->fit[v].ok) continue;
@@ -171,7 +157,7 @@ static int heuristic_variant(const dedisp_plan *pl) {
         double rate, need, occ;
         if (x.kind == KIND_TREE) {
             rate = (tile >= 100 ? (x.threads >= 384 ? 62 : 58) : tile >= 72 ? 52 : 42) *
-                   (pl->dtype == DEDISP_U8 ? 0.85 : 1.0);
+                   (pl->dtype == DEDISP_U8 ? 1.4 : 1.0);  // uint8: two adds per integer add
             need = 8;
             occ = x.threads <= 128 ? 4 : (x.threads <= 256 && tile <= 48) ? 2 : 1;
         } else if (x.kind == KIND_LDS) {
@@ -238,6 +224,7 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     const int al = in_dtype == DEDISP_U8 ? 16 : 4;
     int64_t in_samples;
 
+    CUDA_TRY(cudaGetDevice(&pl->device), "cudaGetDevice");
     CUDA_TRY(cudaMalloc(&pl->d_shift, (size_t)nr_dms * nr_channels * 4), "cudaMalloc(shift)");
     CUDA_TRY(cudaMalloc(&pl->d_shiftT, (size_t)nr_channels * pl->dpitch * 4), "cudaMalloc(shiftT)");
     CUDA_TRY(cudaMalloc(&d_flag, 4), "cudaMalloc(flag)");
@@ -264,11 +251,27 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     in_samples = nr_samples + pl->M;
     if (in_samples + al > INT32_MAX) { status = DEDISP_ERR_OVERFLOW; goto fail; }
     pl->in_pitch = (int)((in_samples + al - 1) / al * al);
-    if (build_tree_tables(pl) != cudaSuccess) goto cuda_fail;
+    // uint8 tree kernels: pair y = samples y and y + S2 of a row (kernel_tree.cuh)
+    pl->S2 = (int)((((nr_samples + 1) / 2) + 3) & ~(int64_t)3);
+    pl->pair_pitch = (int)((pl->S2 + pl->M + 3) & ~(int64_t)3);
+    if (build_tree_slopes(pl) != cudaSuccess) goto cuda_fail;
     compute_fits(pl);
     pl->variant = heuristic_variant(pl);
+    if (pl->variant < 0) {
+        snprintf(g_last_error, sizeof g_last_error,
+                 "no compiled kernel variant supports this plan (nr_dms > 65535 and shifts too long "
+                 "for the staged kernels)");
+        status = DEDISP_ERR_INVALID_ARG;
+        goto fail;
+    }
     if (const char *cache = getenv("DEDISP_TUNE_CACHE"))
-        if (*cache) dedisp_plan_load_tuning(pl, cache);  // missing file / entry: keep the heuristic
+        if (*cache) dedisp_plan_load_tuning(pl, cache, 1, nullptr);  // missing file / entry: keep the heuristic
+    if (in_dtype == DEDISP_U8 && pl->tree.valid) {
+        status = dedisp_plan_reserve(pl, 1);
+        if (status != DEDISP_OK) goto fail;
+    }
+    status = prepare_variant(pl, pl->variant);
+    if (status != DEDISP_OK) goto fail;
     *plan = pl;
     return DEDISP_OK;
 
@@ -278,6 +281,21 @@ fail:
     if (d_flag) cudaFree(d_flag);
     dedisp_plan_destroy(pl);
     return status;
+}
+
+int dedisp_plan_reserve(dedisp_plan *plan, int nr_beams) {
+    if (!plan || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
+    if (plan->dtype != DEDISP_U8 || !plan->tree.valid || nr_beams <= plan->pairs_beams) return DEDISP_OK;
+    // the old workspace may still be read by kernels in flight
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { set_last_error("cudaDeviceSynchronize", e); return DEDISP_ERR_CUDA; }
+    uint32_t *p = nullptr;
+    e = cudaMalloc(&p, (size_t)nr_beams * plan->C * plan->pair_pitch * 4);
+    if (e != cudaSuccess) { set_last_error("cudaMalloc(pair workspace)", e); return DEDISP_ERR_ALLOC; }
+    if (plan->d_pairs) cudaFree(plan->d_pairs);
+    plan->d_pairs = p;
+    plan->pairs_beams = nr_beams;
+    return DEDISP_OK;
 }
 
 int dedisp_shift_table(const dedisp_plan *plan, int32_t *host_out) {
@@ -302,11 +320,13 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value) {
         case DEDISP_NR_SAMPLES: *value = plan->S; break;
         case DEDISP_IN_DTYPE: *value = plan->dtype; break;
         case DEDISP_MAX_STEP: *value = plan->max_step; break;
+        case DEDISP_RESERVED_BEAMS: *value = plan->dtype == DEDISP_U8 ? plan->pairs_beams : 0; break;
         default: return DEDISP_ERR_INVALID_ARG;
     }
     return DEDISP_OK;
 }
 
+// Enqueue variant v for nr_beams beams.  Kernels only: no allocation, no host synchronisation.
 static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void *d_out,
                           int nr_beams, cudaStream_t st) {
     const Variant &x = variants()[v];
@@ -315,52 +335,63 @@ static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void
     a.in = d_in; a.out = d_out; a.shift = plan->d_shift; a.shiftT = plan->d_shiftT;
     a.C = plan->C; a.D = plan->D; a.S = (int)plan->S; a.in_pitch = plan->in_pitch;
     a.dpitch = plan->dpitch; a.lrow = f.lrow;
+    a.pairs = plan->d_pairs; a.pair_pitch = plan->pair_pitch; a.S2 = plan->S2;
+    a.zero = 0; a.one = 1;
     const TreeTable *tt = x.kind == KIND_TREE ? plan->tree.find(x.dt, x.dms_cta) : nullptr;
+    if (x.kind == KIND_TREE && !tt) return DEDISP_ERR_INVALID_ARG;  // variant was never prepared
     a.desc = tt ? tt->d_desc : nullptr;
     a.descpitch = tt ? tt->pitch : 0;
-    // grid.z carries the beams (step a7): at most 65535 per launch
+    // grid.z carries the beams (step a7): at most 65535 per launch; the uint8 tree kernels
+    // go through the pair workspace, as many beams at a time as it was reserved for
+    const bool paired = x.kind == KIND_TREE && plan->dtype == DEDISP_U8;
+    if (paired && (!plan->d_pairs || plan->pairs_beams < 1)) return DEDISP_ERR_INVALID_ARG;
+    const int group = paired ? std::min(plan->pairs_beams, 65535) : 65535;
     const size_t in_beam = (size_t)plan->C * plan->in_pitch * (plan->dtype == DEDISP_U8 ? 1 : 4);
     const size_t out_beam = (size_t)plan->D * plan->S * 4;
-    for (int b0 = 0; b0 < nr_beams; b0 += 65535) {
-        int nb = std::min(65535, nr_beams - b0);
+    for (int b0 = 0; b0 < nr_beams; b0 += group) {
+        int nb = std::min(group, nr_beams - b0);
         a.in = (const char *)d_in + (size_t)b0 * in_beam;
         a.out = (char *)d_out + (size_t)b0 * out_beam;
-        cudaError_t e = x.launch(a, nb, f.smem, st);
+        cudaError_t e = cudaSuccess;
+        if (paired)
+            e = pack_pairs((const uint8_t *)a.in, plan->d_pairs, nb, plan->C, plan->in_pitch,
+                           plan->pair_pitch, plan->S2, st);
+        if (e == cudaSuccess) e = x.launch(a, nb, f.smem, st);
         if (e != cudaSuccess) { set_last_error(x.name, e); return DEDISP_ERR_CUDA; }
     }
     return DEDISP_OK;
 }
 
-// cudaFuncSetAttribute once per (variant, device context); cheap to repeat, so no global state
-// beyond a per-process flag array.
-static int prepare_variant(const dedisp_plan *plan, int v) {
-    static std::mutex mu;
-    static std::vector<size_t> prepared;
-    std::lock_guard<std::mutex> lk(mu);
-    if (prepared.size() != variants().size()) prepared.assign(variants().size(), 0);
-    size_t need = plan->fit[v].smem;
-    if (need <= prepared[v] || need <= 48 * 1024) return DEDISP_OK;
-    cudaError_t e = variants()[v].prepare(need);
-    if (e != cudaSuccess) { set_last_error("cudaFuncSetAttribute", e); return DEDISP_ERR_CUDA; }
-    prepared[v] = need;
+static int check_execute_args(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams) {
+    if (!plan || !d_in || !d_out || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return DEDISP_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != plan->device) {
+        snprintf(g_last_error, sizeof g_last_error,
+                 "the plan lives on device %d but the current device is %d", plan->device, dev);
+        return DEDISP_ERR_INVALID_ARG;
+    }
     return DEDISP_OK;
 }
 
 int dedisp_execute_variant(const dedisp_plan *plan, int variant, const void *d_in, void *d_out,
                            int nr_beams, void *stream) {
-    if (!plan || !d_in || !d_out || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
-    if (((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return DEDISP_ERR_INVALID_ARG;
+    int rc = check_execute_args(plan, d_in, d_out, nr_beams);
+    if (rc != DEDISP_OK) return rc;
     if (variant < 0 || variant >= (int)variants().size() || !plan->fit[variant].ok)
         return DEDISP_ERR_INVALID_ARG;
-    int rc = prepare_variant(plan, variant);
+    // an explicitly chosen variant may not have been selected before: prepare it here (this is the
+    // tuner's and the tests' entry point; dedisp_execute never takes this branch's allocations)
+    rc = prepare_variant(const_cast<dedisp_plan *>(plan), variant);
     if (rc != DEDISP_OK) return rc;
     return launch_variant(plan, variant, d_in, d_out, nr_beams, (cudaStream_t)stream);
 }
 
 int dedisp_execute(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
                    void *stream) {
-    if (!plan) return DEDISP_ERR_INVALID_ARG;
-    return dedisp_execute_variant(plan, plan->variant, d_in, d_out, nr_beams, stream);
+    int rc = check_execute_args(plan, d_in, d_out, nr_beams);
+    if (rc != DEDISP_OK) return rc;
+    return launch_variant(plan, plan->variant, d_in, d_out, nr_beams, (cudaStream_t)stream);
 }
 
 int dedisp_execute_host(dedisp_plan *plan, const void *h_in, void *h_out, int nr_beams,
@@ -397,13 +428,15 @@ int dedisp_execute_host(dedisp_plan *plan, const void *h_in, void *h_out, int nr
 
 int dedisp_plan_destroy(dedisp_plan *plan) {
     if (!plan) return DEDISP_OK;
+    plan->pipe.destroy();  // drains the host pipeline's streams first
     if (plan->d_shift) cudaFree(plan->d_shift);
     if (plan->d_shiftT) cudaFree(plan->d_shiftT);
+    if (plan->tree.d_qc) cudaFree(plan->tree.d_qc);
     for (auto &t : plan->tree.tables)
         if (t.d_desc) cudaFree(t.d_desc);
+    if (plan->d_pairs) cudaFree(plan->d_pairs);
     if (plan->ws_in) cudaFree(plan->ws_in);
     if (plan->ws_out) cudaFree(plan->ws_out);
-    plan->pipe.destroy();
     delete plan;
     return DEDISP_OK;
 }
@@ -422,6 +455,8 @@ int dedisp_variant_supported(const dedisp_plan *plan, int variant) {
 
 int dedisp_plan_set_variant(dedisp_plan *plan, int variant) {
     if (!dedisp_variant_supported(plan, variant)) return DEDISP_ERR_INVALID_ARG;
+    int rc = prepare_variant(plan, variant);
+    if (rc != DEDISP_OK) return rc;
     plan->variant = variant;
     return DEDISP_OK;
 }

@@ -119,6 +119,35 @@ __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, 
     desc[(size_t)c * descpitch + G] = ((uint32_t)woff & 0xffffu) << 16 | (0x100u << q) | bits;
 }
 
+// pack_pairs_kernel: the uint8 tree kernels' view of the input (kernel_tree.cuh).  One thread per four
+// pairs: pairs[b][c][y] = in[b][c][y] | in[b][c][y + S2] << 16, samples past the row read as 0.
+__global__ void pack_pairs_kernel(const uint8_t *in, uint32_t *pairs, int in_pitch, int pair_pitch,
+                                  int S2) {
+    const int y4 = blockIdx.x * blockDim.x + threadIdx.x;  // group of four pairs
+    if (4 * y4 >= pair_pitch) return;
+    const size_t row = blockIdx.y + (size_t)blockIdx.z * gridDim.y;
+    const uint32_t *r = reinterpret_cast<const uint32_t *>(in + row * in_pitch);
+    const int n4 = in_pitch >> 2;  // in_pitch is a multiple of 16
+    const uint32_t lo = y4 < n4 ? r[y4] : 0u;
+    const uint32_t hi = y4 + (S2 >> 2) < n4 ? r[y4 + (S2 >> 2)] : 0u;
+    const uint32_t le = __byte_perm(lo, 0, 0x4240), lq = __byte_perm(lo, 0, 0x4341);
+    const uint32_t he = __byte_perm(hi, 0, 0x4240), hq = __byte_perm(hi, 0, 0x4341);
+    uint4 v;
+    v.x = __byte_perm(le, he, 0x5410);
+    v.y = __byte_perm(lq, hq, 0x5410);
+    v.z = __byte_perm(le, he, 0x7632);
+    v.w = __byte_perm(lq, hq, 0x7632);
+    reinterpret_cast<uint4 *>(pairs + row * pair_pitch)[y4] = v;
+}
+
+cudaError_t pack_pairs(const uint8_t *d_in, uint32_t *d_pairs, int nr_beams, int C, int in_pitch,
+                       int pair_pitch, int S2, cudaStream_t st) {
+    dim3 block(256);
+    dim3 grid((pair_pitch / 4 + 255) / 256, C, nr_beams);
+    pack_pairs_kernel<<<grid, block, 0, st>>>(d_in, d_pairs, in_pitch, pair_pitch, S2);
+    return cudaGetLastError();
+}
+
 cudaError_t build_chan_slopes(const int32_t *d_shiftT, int C, int D, int dpitch, int *d_qc,
                               int *d_flags, cudaStream_t st) {
     chan_slope_kernel<<<C, 128, 0, st>>>(d_shiftT, D, dpitch, d_qc, d_flags);

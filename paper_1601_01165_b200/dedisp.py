@@ -18,11 +18,11 @@ LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
 
 F32, U8 = 0, 1
 (MAX_SHIFT, IN_SAMPLES, IN_PITCH, OUT_PITCH, VARIANT, NR_CHANNELS, NR_DMS, NR_SAMPLES, IN_DTYPE,
- MAX_STEP) = range(10)
+ MAX_STEP, RESERVED_BEAMS) = range(11)
 
 # every symbol include/dedisp.h declares
 SYMBOLS = [
-    "dedisp_plan_create", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
+    "dedisp_plan_create", "dedisp_plan_reserve", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
     "dedisp_execute_variant", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
     "dedisp_stream_block_async",
     "dedisp_plan_destroy", "dedisp_variant_count",
@@ -50,6 +50,7 @@ def load_library() -> ctypes.CDLL:
     lib = ctypes.CDLL(LIB_PATH)
     vp, ci, i64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
     lib.dedisp_plan_create.argtypes = [ctypes.POINTER(vp), ci, dbl, dbl, dbl, i64, dbl, dbl, ci, ci]
+    lib.dedisp_plan_reserve.argtypes = [vp, ci]
     lib.dedisp_shift_table.argtypes = [vp, vp]
     lib.dedisp_plan_get.argtypes = [vp, ci, ctypes.POINTER(i64)]
     lib.dedisp_execute.argtypes = [vp, vp, vp, ci, vp]
@@ -65,7 +66,7 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_variant_supported.argtypes = [vp, ci]
     lib.dedisp_plan_set_variant.argtypes = [vp, ci]
     lib.dedisp_tune.argtypes = [vp, vp, vp, ci, vp, ctypes.c_char_p, vp]
-    lib.dedisp_plan_load_tuning.argtypes = [vp, ctypes.c_char_p]
+    lib.dedisp_plan_load_tuning.argtypes = [vp, ctypes.c_char_p, ci, ctypes.POINTER(ci)]
     lib.dedisp_status_string.argtypes = [ci]
     lib.dedisp_status_string.restype = ctypes.c_char_p
     lib.dedisp_last_error.argtypes = []
@@ -154,6 +155,11 @@ class Plan:
     nr_samples = property(lambda self: self.get(NR_SAMPLES))
     in_dtype = property(lambda self: self.get(IN_DTYPE))
     max_step = property(lambda self: self.get(MAX_STEP))
+    reserved_beams = property(lambda self: self.get(RESERVED_BEAMS))
+
+    def reserve(self, nr_beams: int):
+        """dedisp_plan_reserve: size the uint8 pair workspace for batches of nr_beams beams."""
+        _check(self._lib.dedisp_plan_reserve(self._h, int(nr_beams)), "dedisp_plan_reserve")
 
     def shift_table(self) -> np.ndarray:
         """dedisp_shift_table: int32 [nr_dms][nr_channels], copied from the device table."""
@@ -208,6 +214,9 @@ class Plan:
                                      ms.ctypes.data), "dedisp_tune")
         return {v: float(ms[v]) for v in range(len(ms)) if ms[v] >= 0}
 
-    def load_tuning(self, cache_path: str):
-        _check(self._lib.dedisp_plan_load_tuning(self._h, cache_path.encode()),
-               "dedisp_plan_load_tuning")
+    def load_tuning(self, cache_path: str, nr_beams: int = 1) -> bool:
+        """dedisp_plan_load_tuning: True if the cache had an entry for this setup and it was applied."""
+        hit = ctypes.c_int(0)
+        _check(self._lib.dedisp_plan_load_tuning(self._h, cache_path.encode(), int(nr_beams),
+                                                 ctypes.byref(hit)), "dedisp_plan_load_tuning")
+        return bool(hit.value)

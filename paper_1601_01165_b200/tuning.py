@@ -10,13 +10,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SHIPPED = os.path.join(HERE, "tuned", "b200.tsv")
 
 
-def apply_shipped(plan) -> None:
-    """Select the persisted winner for this plan's setup, if the shipped file has one."""
-    if os.path.exists(SHIPPED):
-        plan.load_tuning(SHIPPED)
+def apply_shipped(plan, nr_beams: int = 1) -> bool:
+    """Select the persisted winner for this plan's setup and batch size, if the shipped file has one.
+    Returns whether an entry was applied (False: the plan keeps its cost-model default)."""
+    return os.path.exists(SHIPPED) and plan.load_tuning(SHIPPED, nr_beams)
 
 
-def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 4) -> None:
+def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 8) -> None:
     import torch
 
     from . import dedisp, workloads as wl
@@ -31,6 +31,7 @@ def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 4) -> None:
         in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
         d_in = torch.zeros((nb, s.nr_channels, plan.in_pitch), dtype=in_dt, device="cuda")
         d_out = torch.empty((nb, s.nr_dms, s.nr_samples), dtype=torch.float32, device="cuda")
+        plan.reserve(nb)
         ms = plan.tune(d_in, d_out, nr_beams=nb, cache_path=tmp)
         for v, t in sorted(ms.items(), key=lambda kv: kv[1]):
             print("%-10s %9.4f ms  %s" % (name, t, dedisp.variant_name(v)))

@@ -19,11 +19,11 @@ spec.loader.exec_module(gen_tree)
 def parse_lattice(text, q):
     """{label: (j, r, {bit value: next label})} of run_q<q>, and its window length."""
     body = text.split("void run_q%d(" % q)[1].split("DONE:;")[0]
-    wlen = int(re.search(r"float w\[(\d+)\];", body).group(1))
+    wlen = int(re.search(r"(?:float|uint32_t) w\[(\d+)\];", body).group(1))
     loads = len(re.findall(r"v = p4\[\d+\];", body))
     assert loads * 4 == wlen
     nodes = {}
-    for m in re.finditer(r"N_(\d+)_(\d+):\s*\n\s*tree_add<(\d+), (\d+)>\(acc\[(\d+)\], w\);\s*\n\s*(.*)", body):
+    for m in re.finditer(r"N_(\d+)_(\d+):\s*\n\s*tree_add<(\d+), (\d+)>\(acc\[(\d+)\], w(?:, zero, one)?\);\s*\n\s*(.*)", body):
         j, r, radd, tt, jacc, tail = int(m[1]), int(m[2]), int(m[3]), int(m[4]), int(m[5]), m[6]
         assert r == radd and j == jacc
         t = re.match(r"if \(bits & (\d+)u\) goto (N_\d+_\d+); else goto (N_\d+_\d+);", tail)
@@ -38,9 +38,11 @@ def parse_lattice(text, q):
     return nodes, wlen, {3: entry[1], 2: entry[2], 1: entry[3], 0: entry[4]}
 
 
-@pytest.mark.parametrize("dt,tt,qmax", [(4, 28, 3), (6, 28, 4), (8, 20, 3), (4, 12, 4)])
-def test_lattice_walk_visits_the_right_offsets(dt, tt, qmax):
-    text = gen_tree.emit(dt, tt, qmax)
+@pytest.mark.parametrize("dt,tt,qmax,typ", [(4, 28, 3, "f32"), (6, 28, 4, "f32"), (8, 20, 3, "f32"),
+                                            (4, 12, 4, "f32"), (4, 28, 4, "u32"), (5, 20, 4, "u32")])
+def test_lattice_walk_visits_the_right_offsets(dt, tt, qmax, typ):
+    text = gen_tree.emit(dt, tt, qmax, typ)
+    assert "struct TreeStep<%s, %d, %d, %d>" % (gen_tree.CTYPE[typ][0], dt, tt, qmax) in text
     assert "WNMAX = %d" % gen_tree.wn(dt, tt, qmax) in text
     for q in range(qmax + 1):
         nodes, wlen, entry = parse_lattice(text, q)
@@ -71,3 +73,25 @@ def test_chunk_loop_dispatches_one_hot_slope_classes():
         assert "if (d & %du) goto L%d;" % (0x100 << q, q) in chunk
         assert "run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu);" % q in chunk
     assert "goto L3;" in chunk
+    # the uint8 lattices carry the two run-time constants that pin the pipe of each add
+    chunk = gen_tree.emit(4, 28, 4, "u32").split("void chunk(")[1]
+    assert "uint32_t zero, uint32_t one" in chunk
+    assert "run_q4(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu, zero, one);" in chunk
+
+
+def test_variant_list_is_the_single_source_of_the_registry():
+    """csrc/variants.py is the one place a variant is added: the generated registry
+    has one maker per entry, in list order, generic first."""
+    from paper_1601_01165_b200 import build
+    v = build._variants()
+    units = v.units()
+    assert [n for n, _ in units[:2]] == ["generic0", "generic1"]
+    assert len(units) == len(v.GENERIC) + len(v.LDS) + len(v.TREE)
+    assert len(set(e for _, e in units)) == len(units), "duplicate variant"
+    build.generate()
+    inc = open(os.path.join(build.OBJ, "registry_gen.inc")).read()
+    assert [m for m in re.findall(r"^    variant_(\w+),$", inc, flags=re.M)] == [n for n, _ in units]
+    for t in v.TREE:
+        typ = "u32" if t[0] == "uint8_t" else "f32"
+        assert "%s:%d,%d,%d" % (typ, t[3], t[4], t[7]) in v.tree_combos()
+        assert t[4] % 4 == 0 and (t[4] // 4) % 2 == 1, "TT/4 odd keeps LDS.128 conflict-free"
