@@ -36,10 +36,12 @@ void HostPipe::destroy() {
 static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
     cudaError_t e = cudaSuccess;
     if (!p.ready) {
+        // a half-built pipeline is torn down again: the next call starts from scratch, nothing leaks
         if ((e = cudaStreamCreateWithFlags(&p.s_h2d, cudaStreamNonBlocking)) != cudaSuccess ||
             (e = cudaStreamCreateWithFlags(&p.s_exec, cudaStreamNonBlocking)) != cudaSuccess ||
             (e = cudaStreamCreateWithFlags(&p.s_d2h, cudaStreamNonBlocking)) != cudaSuccess) {
             set_last_error("cudaStreamCreate", e);
+            p.destroy();
             return DEDISP_ERR_CUDA;
         }
         for (int i = 0; i < HostPipe::kSlots; ++i)
@@ -47,6 +49,7 @@ static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
                 (e = cudaEventCreateWithFlags(&p.ev_exec[i], cudaEventDisableTiming)) != cudaSuccess ||
                 (e = cudaEventCreateWithFlags(&p.ev_out[i], cudaEventDisableTiming)) != cudaSuccess) {
                 set_last_error("cudaEventCreate", e);
+                p.destroy();
                 return DEDISP_ERR_CUDA;
             }
         p.ready = true;
@@ -69,7 +72,7 @@ static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
         }
         if (e != cudaSuccess) {
             set_last_error("cudaMalloc(host pipeline workspace)", e);
-            p.in_bytes = p.out_bytes = 0;
+            p.destroy();
             return DEDISP_ERR_ALLOC;
         }
         if (in_bytes > p.in_bytes) p.in_bytes = in_bytes;
@@ -86,6 +89,23 @@ static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
         if (e_ != cudaSuccess) {               \
             set_last_error(what, e_);          \
             return DEDISP_ERR_CUDA;            \
+        }                                      \
+    } while (0)
+
+// A failure in the middle of a pipelined call leaves copies and events of this slot enqueued without
+// the ordering a later reuse of the slot relies on: drain the three streams before reporting it.
+static int pipe_abort(dedisp::HostPipe &p, int rc) {
+    cudaStreamSynchronize(p.s_h2d);
+    cudaStreamSynchronize(p.s_exec);
+    cudaStreamSynchronize(p.s_d2h);
+    return rc;
+}
+#define PIPE_TRY_DRAIN(expr, what)             \
+    do {                                       \
+        cudaError_t e_ = (expr);               \
+        if (e_ != cudaSuccess) {               \
+            set_last_error(what, e_);          \
+            return pipe_abort(p, DEDISP_ERR_CUDA); \
         }                                      \
     } while (0)
 
@@ -112,22 +132,22 @@ static int pipe_call(dedisp_plan *plan, const void *h_in, void *h_out, int nr_be
                                    (const char *)h_in + (size_t)t0 * esz, (size_t)series_pitch * esz,
                                    (size_t)(plan->S + plan->M) * esz, (size_t)plan->C,
                                    cudaMemcpyHostToDevice, p.s_h2d), "H2D (2-D)");
-    PIPE_TRY(cudaEventRecord(p.ev_in[s], p.s_h2d), "cudaEventRecord");
+    PIPE_TRY_DRAIN(cudaEventRecord(p.ev_in[s], p.s_h2d), "cudaEventRecord");
     // stage 2: the kernels, once the input is there and the slot's previous output has left
-    PIPE_TRY(cudaStreamWaitEvent(p.s_exec, p.ev_in[s], 0), "cudaStreamWaitEvent");
-    if (reused) PIPE_TRY(cudaStreamWaitEvent(p.s_exec, p.ev_out[s], 0), "cudaStreamWaitEvent");
+    PIPE_TRY_DRAIN(cudaStreamWaitEvent(p.s_exec, p.ev_in[s], 0), "cudaStreamWaitEvent");
+    if (reused) PIPE_TRY_DRAIN(cudaStreamWaitEvent(p.s_exec, p.ev_out[s], 0), "cudaStreamWaitEvent");
     rc = dedisp_execute(plan, p.in[s], p.out[s], nr_beams, p.s_exec);
-    if (rc != DEDISP_OK) return rc;
-    PIPE_TRY(cudaEventRecord(p.ev_exec[s], p.s_exec), "cudaEventRecord");
+    if (rc != DEDISP_OK) return pipe_abort(p, rc);
+    PIPE_TRY_DRAIN(cudaEventRecord(p.ev_exec[s], p.s_exec), "cudaEventRecord");
     // stage 3: D2H
-    PIPE_TRY(cudaStreamWaitEvent(p.s_d2h, p.ev_exec[s], 0), "cudaStreamWaitEvent");
+    PIPE_TRY_DRAIN(cudaStreamWaitEvent(p.s_d2h, p.ev_exec[s], 0), "cudaStreamWaitEvent");
     if (series_pitch == 0)
-        PIPE_TRY(cudaMemcpyAsync(h_out, p.out[s], out_bytes, cudaMemcpyDeviceToHost, p.s_d2h), "D2H");
+        PIPE_TRY_DRAIN(cudaMemcpyAsync(h_out, p.out[s], out_bytes, cudaMemcpyDeviceToHost, p.s_d2h), "D2H");
     else
-        PIPE_TRY(cudaMemcpy2DAsync((char *)h_out + (size_t)t0 * 4, (size_t)out_pitch * 4, p.out[s],
+        PIPE_TRY_DRAIN(cudaMemcpy2DAsync((char *)h_out + (size_t)t0 * 4, (size_t)out_pitch * 4, p.out[s],
                                    (size_t)plan->S * 4, (size_t)plan->S * 4, (size_t)plan->D,
                                    cudaMemcpyDeviceToHost, p.s_d2h), "D2H (2-D)");
-    PIPE_TRY(cudaEventRecord(p.ev_out[s], p.s_d2h), "cudaEventRecord");
+    PIPE_TRY_DRAIN(cudaEventRecord(p.ev_out[s], p.s_d2h), "cudaEventRecord");
     ++p.calls;
     return DEDISP_OK;
 }

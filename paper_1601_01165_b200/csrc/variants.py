@@ -85,6 +85,14 @@ TREE = [
     ("uint8_t", 12, 1, 4, 28, 8, 3, 4, 1),  # 48 x 1792, 12 warps
     ("uint8_t", 12, 1, 4, 28, 8, 2, 4, 1),
     ("uint8_t", 12, 1, 4, 20, 8, 3, 4, 1),  # 48 x 1280
+    ("uint8_t", 12, 1, 4, 20, 16, 3, 4, 1),
+    ("uint8_t", 12, 1, 4, 20, 12, 4, 4, 1),
+    ("uint8_t", 12, 1, 4, 20, 8, 4, 4, 1),
+    ("uint8_t", 12, 1, 4, 28, 16, 2, 4, 1),
+    ("uint8_t", 12, 1, 4, 28, 12, 3, 4, 1),
+    ("uint8_t", 12, 1, 5, 20, 16, 3, 4, 1),
+    ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1),
+    ("uint8_t", 16, 1, 4, 12, 16, 3, 4, 1),
     ("uint8_t", 12, 1, 5, 20, 8, 3, 4, 1),  # 60 x 1280
     ("uint8_t", 12, 1, 6, 12, 8, 3, 4, 1),  # 72 x 768
     ("uint8_t", 16, 1, 5, 12, 8, 3, 4, 1),  # 80 x 768, 16 warps

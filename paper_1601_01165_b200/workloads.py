@@ -84,7 +84,9 @@ def make_input(setup: Setup, in_samples: int, in_pitch: int,
                pulse_shifts: Optional[np.ndarray] = None,
                beams: Optional[range] = None) -> np.ndarray:
     """Seeded input [B][C][in_pitch]; samples [0, in_samples) of every row are
-    drawn from the RNG (nothing is zero-filled: reading A8), the pitch padding is 0.
+    drawn from the RNG (nothing is zero-filled: reading A8).  The pitch padding is
+    POISONED (NaN for fp32, 255 for uint8): the contract says it is ignored, so a
+    kernel that lets it reach an output shows up in every parity test.
 
     Beam b of a multi-beam setup uses seed + b, so any subset of beams can be
     regenerated.  pulse_shifts: int array [C], the shifts of setup.pulse's DM row,
@@ -93,7 +95,8 @@ def make_input(setup: Setup, in_samples: int, in_pitch: int,
     assert in_pitch >= in_samples
     beams = range(setup.nr_beams) if beams is None else beams
     C = setup.nr_channels
-    x = np.zeros((len(beams), C, in_pitch), dtype=setup.np_in_dtype)
+    x = np.full((len(beams), C, in_pitch), 255 if setup.in_dtype == U8 else np.nan,
+                dtype=setup.np_in_dtype)
     for k, b in enumerate(beams):
         rng = np.random.default_rng(setup.seed + b)
         if setup.values == "gauss":

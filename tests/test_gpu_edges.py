@@ -74,6 +74,76 @@ def test_execute_is_repeatable_and_stream_ordered(dd):
     plan.destroy()
 
 
+@pytest.mark.parametrize("u8", [False, True])
+def test_first_execute_of_a_fresh_plan_can_be_captured_into_a_cuda_graph(dd, u8):
+    """dedisp_execute promises no allocation, no host sync and no function-attribute call (all done
+    when the variant is selected): the FIRST call on a fresh plan is captured into a CUDA graph and
+    the replays are bit-exact against the oracle (include/dedisp.h)."""
+    import torch
+    s = wl.scaled(wl.SURVEY8 if u8 else wl.APERTIF, name="graph", nr_channels=300,
+                  channel_bw_MHz=300.0 / 300, nr_dms=150, nr_samples=4100, nr_beams=2,
+                  values="u8" if u8 else "int16", in_dtype=wl.U8 if u8 else wl.F32)
+    plan, table, x, d_in = make_case(dd, s)
+    # a kernel that needs everything a selection prepares: > 48 KB of dynamic shared memory, a
+    # descriptor table and (uint8) the pair workspace
+    tree = [v for v in plan.supported_variants() if dd.variant_name(v).startswith("tree_")]
+    plan.set_variant(tree[0])
+    if u8:
+        plan.reserve(s.nr_beams)
+    ref = oracle.dedisperse(x, table, s.nr_samples)
+    d_out = out_buffer(s, fill=-1)
+    st = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(graph, stream=st):
+        plan.execute(d_in, d_out, nr_beams=s.nr_beams, stream=torch.cuda.current_stream())
+    for _ in range(2):
+        d_out.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        got = to_host(s, d_out)
+        assert np.array_equal(got.astype(np.uint64 if u8 else np.float64), ref)
+    plan.destroy()
+
+
+def test_u8_batches_larger_than_the_reserved_workspace(dd):
+    """A uint8 plan reserves its pair workspace for one beam; a larger batch goes through it one group
+    at a time, and after dedisp_plan_reserve in one launch: same bits either way."""
+    import torch
+    s = wl.Setup("resv", 40, 1400.0, 3.0, 20000.0, 2100, 0.0, 0.25, 70, nr_beams=5, in_dtype=wl.U8,
+                 values="u8", seed=21)
+    plan, table, x, d_in = make_case(dd, s)
+    ref = oracle.dedisperse(x, table, s.nr_samples)
+    tv = [v for v in plan.supported_variants() if dd.variant_name(v).startswith("tree_u8")]
+    assert tv and plan.reserved_beams == 1
+    for resv in (1, 2, 5):
+        plan.reserve(resv)
+        assert plan.reserved_beams == max(resv, 1)
+        d_out = out_buffer(s, fill=-1)
+        plan.execute_variant(tv[0], d_in, d_out, nr_beams=s.nr_beams)
+        assert np.array_equal(to_host(s, d_out).astype(np.uint64), ref), "reserved %d" % resv
+    with dd.Plan(*wl.TINY.plan_args()) as f32:
+        f32.reserve(4)
+        assert f32.reserved_beams == 0      # fp32 plans have no workspace
+    plan.destroy()
+
+
+def test_execute_on_another_device_is_refused(dd):
+    """The plan belongs to the device it was created on: with one GPU this can only check
+    that the current device is accepted and that the plan reports a mismatch cleanly if there are two."""
+    import torch
+    s = wl.TINY
+    plan, table, x, d_in = make_case(dd, s)
+    d_out = out_buffer(s)
+    plan.execute(d_in, d_out)
+    if torch.cuda.device_count() > 1:
+        with torch.cuda.device(1):
+            with pytest.raises(dd.DedispError) as e:
+                plan.execute(d_in, d_out)
+            assert e.value.status == 1
+    plan.destroy()
+
+
 def test_execute_host_matches_device_path(dd):
     import torch
     s = wl.scaled(wl.APERTIF, name="host", nr_channels=64, channel_bw_MHz=300.0 / 64, nr_dms=64,
@@ -191,12 +261,23 @@ def test_tuner_selects_persists_and_reloads(dd, tmp_path):
     # a fresh plan picks the winner up from the cache; another setup is left alone
     with dd.Plan(*s.plan_args()) as p2:
         p2.set_variant(0)
-        p2.load_tuning(cache)
+        assert p2.load_tuning(cache) is True
         assert p2.variant == best
     with dd.Plan(*wl.TINY.plan_args()) as p3:
         before = p3.variant
-        p3.load_tuning(cache)
+        assert p3.load_tuning(cache) is False
         assert p3.variant == before
+    # the key carries a batch-size class (1 / 2-7 / >= 8 beams): a 40-beam winner does not overwrite the
+    # single-beam one; a class without an entry falls back to one that has
+    other = [v for v in plan.supported_variants() if v != best][0]
+    line = open(cache).read().splitlines()[-1]
+    assert ";beams=1\t" in line
+    with open(cache, "a") as f:
+        f.write(line.replace(";beams=1\t", ";beams=8\t").replace(dd.variant_name(best), dd.variant_name(other)) + "\n")
+    with dd.Plan(*s.plan_args()) as p4:
+        assert p4.load_tuning(cache, nr_beams=40) and p4.variant == other
+        assert p4.load_tuning(cache, nr_beams=1) and p4.variant == best
+        assert p4.load_tuning(cache, nr_beams=3) and p4.variant in (best, other)
     with pytest.raises(dd.DedispError) as e:
         plan.load_tuning(str(tmp_path / "missing.tsv"))
     assert e.value.status == 5

@@ -292,7 +292,9 @@ def test_injected_pulse_peaks_at_its_dm_and_time():
     pitch = 1036
     x = wl.make_input(s, s.nr_samples + M, pitch, pulse_shifts=t[64])
     noise = wl.make_input(wl.scaled(s, pulse=None), s.nr_samples + M, pitch)
-    assert x.max() <= 115 and np.array_equal(x, np.round(x))
+    valid = x[..., :s.nr_samples + M]           # the pitch padding is poisoned and never read
+    assert valid.max() <= 115 and np.array_equal(valid, np.round(valid))
+    assert np.isnan(x[..., s.nr_samples + M:]).all()
     out = oracle.dedisperse(x, t, s.nr_samples)[0]
     assert np.unravel_index(np.argmax(out), out.shape) == (64, 300)
     assert (out == out.max()).sum() == 1
