@@ -2,13 +2,17 @@
 """bench.py -- dedispersion throughput on B200 (BASELINE.json metric).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config apertif] [--impl ours|reference]
+                  [--only] [--variant V] [--tune] [--no-cpu-baseline]
 
-A step is one pass of the whole hot path (dedisp_execute: staging, shifted accumulate, store) over
-one synthetic batch of the named config.  `value` is dedispersion GFLOP/s = B*D*C*S adds / s
- with inputs resident in HBM; `e2e` is the same through dedisp_execute_host with
-pinned HOST buffers (H2D + kernel + D2H inside the timed region).  The path does not shard
-(replicas only): with --gpus N every rank runs the same workload on its own GPU,
-no collective on the data path, value = all ranks' adds / max-over-ranks time.
+A step is one pass of the whole hot path (dedisp_execute: staging, shifted accumulate, store; for
+uint8 input also the pair repacking) over one synthetic batch of the named config.  `value` is
+dedispersion GFLOP/s = B*D*C*S adds / s with inputs resident in HBM; `e2e` is the
+same through dedisp_execute_host_async with pinned HOST buffers (H2D + kernels + D2H inside the timed
+region).  The default run also times the other four BASELINE.json configs with the same event
+protocol and reports them under `configs` (north star: real-time factor and beams in real time per
+config); --only skips them.  The path does not shard (replicas only): with --gpus N
+every rank runs the same workload on its own GPU, no collective on the data path, value = all ranks'
+adds / max-over-ranks time.
 """
 from __future__ import annotations
 
@@ -31,14 +35,13 @@ METRIC = "dedispersion GFLOP/s"
 UNIT = "GFLOP/s"
 SM_COUNT = 148
 FP32_LANES_PER_SM = 128          # fp32 add issue: 4 SMSPs x 32 lanes per clock
+INT_LANES_PER_SM = 128           # 32-bit integer adds: 64 lanes on the integer pipe + 64 (IMAD) on the FMA pipe
+LDS_WORDS_PER_SM = 32            # shared memory: 128 bytes per clock and SM
 FALLBACK_HBM_GBS = 6650.0        # B200_PROFILING.md fallback
 FALLBACK_SM_MHZ = 1965.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the
-# same command (profiles/README.md says which file); None until captured for that config.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_tree_apertif.md: 114.9 MB read + 123.9 MB written per launch
-    "apertif": 114913536 + 123922432,
-}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full captures summarised
+# under profiles/ (the JSON names the file each number comes from)
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 
 
 def measured_peaks():
@@ -52,14 +55,44 @@ def measured_peaks():
     return FALLBACK_HBM_GBS, FALLBACK_SM_MHZ, "fallback"
 
 
+def ncu_traffic(config_name, variant_name):
+    """(bytes per step, source) for the config if profiles/ holds a capture of this variant."""
+    try:
+        d = json.load(open(TRAFFIC_JSON))[config_name]
+    except Exception:
+        return None, None
+    if d.get("variant") and d["variant"] != variant_name:
+        return None, "profiles capture is of another variant: " + d["variant"]
+    return d["dram_bytes_per_step"], d["source"]
+
+
 def compulsory_bytes(s, in_samples):
     """Input read once + output written once (north_star)."""
     esz = 1 if s.in_dtype == wl.U8 else 4
     return s.nr_beams * (s.nr_channels * in_samples * esz + s.nr_dms * s.nr_samples * 4)
 
 
+def binding_roof(vname, s, sm_max_mhz):
+    """The on-chip roof that bounds the variant's kind of kernel, in T adds/s
+    at the maximum SM clock: (bound, peak, note)."""
+    clk = sm_max_mhz * 1e6
+    if vname.startswith("tree_u8"):
+        return ("alu", SM_COUNT * INT_LANES_PER_SM * 2 * clk / 1e12,
+                "packed 16-bit adds: 148 SMs x 128 integer-add lanes (64 IADD3 + 64 IMAD) x 2 counters "
+                "per 32-bit add x %.0f MHz; a pure add stream measures 115 of the 128 lanes" % sm_max_mhz)
+    if vname.startswith("tree_"):
+        return ("alu", SM_COUNT * FP32_LANES_PER_SM * clk / 1e12,
+                "fp32 adds: 148 SMs x 128 lanes x %.0f MHz max SM clock" % sm_max_mhz)
+    if vname.startswith("lds_"):
+        return ("lds", SM_COUNT * LDS_WORDS_PER_SM * clk / 1e12,
+                "one shared-memory word per add: 148 SMs x 32 words/clk x %.0f MHz (shared-memory "
+                "wavefronts, not an ALU pipe, bind this kind: profiles/r02_ncu_lds_lofar.md)" % sm_max_mhz)
+    return ("l2", SM_COUNT * 10 * clk / 1e12,
+            "no-reuse kernel: about 10 four-byte L2 loads per clk and SM (measured, DESIGN.md section 8)")
+
+
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    """nvidia-smi clocks / throttle reasons DURING the load (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -69,7 +102,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             pass
@@ -85,7 +118,7 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             parts = [x.strip() for x in line.split(",")]
@@ -94,6 +127,7 @@ class ClockSampler:
             try:
                 sm.append(float(parts[0]))
                 mx.append(float(parts[1]))
+                pw.append(float(parts[2]))
             except ValueError:
                 continue
             for n, v in zip(names, parts[3:7]):
@@ -102,7 +136,8 @@ class ClockSampler:
         self.f.close()
         os.unlink(self.f.name)
         if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm),
+                       sm_mhz_min=float(min(sm)), power_w_max=float(max(pw)))
         out["reasons"] = sorted(reasons)
         return out
 
@@ -121,6 +156,15 @@ def max_over_ranks(x: float, world: int, device="cuda") -> float:
 def aggregate_value(adds_per_rank: int, world: int, seconds_max: float) -> float:
     """Whole-job GFLOP/s: every rank processed the same number of adds (weak scaling)."""
     return world * adds_per_rank / seconds_max / 1e9
+
+
+def check_world(gpus: int, world: int) -> None:
+    """--gpus N must agree with the launcher: the driver starts N ranks with torchrun; a bare
+    `python bench.py --gpus 8` would silently measure one GPU."""
+    if gpus != world:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d: launch with `python -m torch.distributed.run "
+                         "--nnodes=1 --nproc-per-node %d --master-addr 127.0.0.1 bench.py --gpus %d ...`"
+                         % (gpus, world, gpus, gpus))
 
 
 def cpu_baseline(s, target_s: float = 12.0):
@@ -149,7 +193,7 @@ def cpu_baseline(s, target_s: float = 12.0):
     adds = len(rows) * s.nr_channels * s.nr_samples
     return {"value": adds / t / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": "%d of %d DM rows (evenly spaced) x %d channels x %d samples, 1 beam, %.1f s"
-                      % (len(rows), D, s.nr_channels, s.nr_samples, t)}, (x, table)
+                      % (len(rows), D, s.nr_channels, s.nr_samples, t)}
 
 
 def run_reference(args, s):
@@ -205,15 +249,117 @@ def workload_name(s):
                             s.channel_bw_MHz, s.sample_rate, s.dm_step))
 
 
+class Case:
+    """One config on the device: plan, rotating synthetic buffer sets, the selected variant."""
+
+    def __init__(self, s, rank, variant=None, tune=False):
+        import torch
+
+        from paper_1601_01165_b200 import dedisp, tuning
+        self.s = s
+        self.plan = plan = dedisp.Plan(*s.plan_args())
+        B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
+        self.in_samples, self.pitch = plan.in_samples, plan.in_pitch
+        self.in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
+        self.out_dt = torch.int32 if s.in_dtype == wl.U8 else torch.float32
+        esz = 1 if s.in_dtype == wl.U8 else 4
+        # Rotating buffer sets so consecutive steps do not find their input in L2 (126 MB).
+        self.set_bytes = B * (C * self.pitch * esz + D * S * 4)
+        self.nbuf = max(2, min(4, int(np.ceil(400e6 / self.set_bytes)) + 1)) if self.set_bytes < 8e9 else 1
+        gen = torch.Generator(device="cuda").manual_seed(s.seed + rank)
+        self.ins, self.outs = [], []
+        for _ in range(self.nbuf):
+            if s.in_dtype == wl.U8:
+                x = torch.randint(0, 256, (B, C, self.pitch), dtype=torch.uint8, device="cuda", generator=gen)
+            else:
+                x = torch.randn((B, C, self.pitch), dtype=torch.float32, device="cuda", generator=gen)
+            self.ins.append(x)
+            self.outs.append(torch.empty((B, D, S), dtype=self.out_dt, device="cuda"))
+        plan.reserve(B)  # uint8: the whole batch in one launch
+        # Auto-tuning (step a8) happens before and outside the timed region.
+        if variant is not None:
+            plan.set_variant(variant)
+            self.tuned = "forced"
+        elif tune:
+            plan.tune(self.ins[0], self.outs[0], nr_beams=B)
+            self.tuned = "dedisp_tune in this run"
+        else:
+            self.tuned = "shipped cache" if tuning.apply_shipped(plan, nr_beams=B) else "heuristic (no cache entry)"
+        self.vname = dedisp.variant_name(plan.variant)
+        # kernels launched per step: the dedispersion kernel, for uint8 tree variants also the repacking
+        self.launches_per_step = 2 if self.vname.startswith("tree_u8") else 1
+
+    def step(self, i, stream):
+        self.plan.execute(self.ins[i % self.nbuf], self.outs[i % self.nbuf], nr_beams=self.s.nr_beams,
+                          stream=stream)
+
+    def close(self):
+        self.plan.destroy()
+        self.ins = self.outs = None
+
+
+def time_device(case, steps, warmup, barrier, min_warm_s=0.0):
+    """W warm-up steps (at least min_warm_s seconds of back-to-back launches), then K steps timed with
+    CUDA events on the launching stream.  Returns (total ms, sorted per-step ms)."""
+    import torch
+    stream = torch.cuda.current_stream()
+    t0 = time.perf_counter()
+    i = 0
+    while i < warmup or (time.perf_counter() - t0) < min_warm_s:
+        case.step(i, stream)
+        i += 1
+        if i % 8 == 0:
+            torch.cuda.synchronize()
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for k in range(steps):
+        case.step(k, stream)
+        ev[k + 1].record(stream)
+    barrier()
+    return ev[0].elapsed_time(ev[-1]), sorted(ev[k].elapsed_time(ev[k + 1]) for k in range(steps))
+
+
+def report(case, world, total_ms, per, steps, hbm_gbs, sm_max_mhz, peak_kind):
+    """The per-config numbers the north star asks for."""
+    s = case.s
+    B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
+    ms_step = total_ms / steps
+    adds = B * D * C * S
+    kern_ms = float(np.mean(per))
+    comp = compulsory_bytes(s, case.in_samples)
+    bound, peak, note = binding_roof(case.vname, s, sm_max_mhz)
+    achieved = adds / (kern_ms * 1e-3) / 1e12
+    traffic, src = ncu_traffic(s.name, case.vname)
+    rt = (S / s.sample_rate) / (ms_step * 1e-3 / B)
+    return {
+        "workload": workload_name(s), "variant": case.vname, "tuning": case.tuned,
+        "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per)), "ms_per_step_min": float(per[0]),
+        "value": aggregate_value(adds, world, ms_step * 1e-3), "unit": UNIT, "dtype": dtype_name(s),
+        "real_time_factor": rt, "beams_in_real_time": int(np.floor(rt)),
+        "beams_memory_cap": int(180e9 // (case.set_bytes / B)),
+        "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": src, "note": note},
+        "hbm_roofline": {"compulsory_bytes": comp, "achieved_gbs": comp / (kern_ms * 1e-3) / 1e9,
+                         "peak_gbs": hbm_gbs, "peak_kind": peak_kind,
+                         "frac": comp / (kern_ms * 1e-3) / 1e9 / hbm_gbs,
+                         "frac_of_nominal_8TBs": comp / (kern_ms * 1e-3) / 8e12},
+        "gpu_launches": steps * case.launches_per_step,
+        "l2": "rotating %d input/output buffer sets (%.0f MB) > 126 MB L2"
+              % (case.nbuf, case.nbuf * case.set_bytes / 1e6),
+    }
+
+
 def run_ours(args, s):
     import torch
     import torch.distributed as dist
 
-    from paper_1601_01165_b200 import build, dedisp, tuning
+    from paper_1601_01165_b200 import build
 
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    check_world(args.gpus, world)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local)
@@ -221,73 +367,31 @@ def run_ours(args, s):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     build.build()
     hbm_gbs, sm_max_mhz, peak_kind = measured_peaks()
-
-    plan = dedisp.Plan(*s.plan_args())
-    in_samples, pitch = plan.in_samples, plan.in_pitch
-    B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
-    in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
-    out_dt = torch.int32 if s.in_dtype == wl.U8 else torch.float32
-    # Rotating buffer sets so consecutive steps do not find their input in L2 (126 MB).
-    esz = 1 if s.in_dtype == wl.U8 else 4
-    set_bytes = B * (C * pitch * esz + D * S * 4)
-    nbuf = max(2, min(4, int(np.ceil(400e6 / set_bytes)) + 1)) if set_bytes < 8e9 else 1
-    gen = torch.Generator(device="cuda").manual_seed(s.seed + rank)
-    ins, outs = [], []
-    for _ in range(nbuf):
-        if s.in_dtype == wl.U8:
-            x = torch.randint(0, 256, (B, C, pitch), dtype=torch.uint8, device="cuda", generator=gen)
-        else:
-            x = torch.randn((B, C, pitch), dtype=torch.float32, device="cuda", generator=gen)
-        ins.append(x)
-        outs.append(torch.empty((B, D, S), dtype=out_dt, device="cuda"))
-
-    # Auto-tuning (step a8) happens before and outside the timed region.
-    tuned = "heuristic"
-    if args.variant is not None:
-        plan.set_variant(args.variant)
-        tuned = "forced"
-    elif args.tune:
-        plan.tune(ins[0], outs[0], nr_beams=B)
-        tuned = "dedisp_tune in this run"
-    else:
-        before = plan.variant
-        tuning.apply_shipped(plan)
-        tuned = "shipped cache" if (os.path.exists(tuning.SHIPPED)) else "heuristic"
-        del before
-    vname = dedisp.variant_name(plan.variant)
-
-    stream = torch.cuda.current_stream()
+    warmup = max(args.warmup, 3)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for i in range(max(args.warmup, 3)):
-        plan.execute(ins[i % nbuf], outs[i % nbuf], nr_beams=B, stream=stream)
-    barrier()
+    case = Case(s, rank, variant=args.variant, tune=args.tune)
+    B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
+    # clocks are sampled over the warm-up (at least 0.6 s of back-to-back launches) and the timed steps
     sampler = ClockSampler(local) if rank == 0 else None
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    barrier()
-    ev[0].record(stream)
-    for i in range(args.steps):
-        plan.execute(ins[i % nbuf], outs[i % nbuf], nr_beams=B, stream=stream)
-        ev[i + 1].record(stream)
-    barrier()
-    total_ms = ev[0].elapsed_time(ev[-1])
-    per = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps))
+    total_ms, per = time_device(case, args.steps, warmup, barrier, min_warm_s=0.6)
     clocks = sampler.stop() if sampler else None
     total_ms = max_over_ranks(total_ms, world)
-    ms_step = total_ms / args.steps
+    head = report(case, world, total_ms, per, args.steps, hbm_gbs, sm_max_mhz, peak_kind)
 
     # ---- end to end through the host-buffer entry point (pinned host memory): every step uploads
     # its input, runs the kernels and downloads its result; consecutive steps overlap on the library's
     # three-stream pipeline (dedisp_execute_host_async), as a streaming real-time user would run it.
-    nslot = 3 if set_bytes < 4e9 else 1
-    h_ins = [torch.empty((B, C, pitch), dtype=in_dt).pin_memory() for _ in range(nslot)]
-    h_outs = [torch.empty((B, D, S), dtype=out_dt).pin_memory() for _ in range(nslot)]
+    plan, pitch = case.plan, case.pitch
+    nslot = 3 if case.set_bytes < 4e9 else 1
+    h_ins = [torch.empty((B, C, pitch), dtype=case.in_dt).pin_memory() for _ in range(nslot)]
+    h_outs = [torch.empty((B, D, S), dtype=case.out_dt).pin_memory() for _ in range(nslot)]
     for h in h_ins:
-        h.copy_(ins[0])
+        h.copy_(case.ins[0])
     e2e_steps = max(3, min(args.steps, 12))
     for i in range(3):
         plan.execute_host_async(h_ins[i % nslot], h_outs[i % nslot], nr_beams=B)
@@ -298,57 +402,65 @@ def run_ours(args, s):
         plan.execute_host_async(h_ins[i % nslot], h_outs[i % nslot], nr_beams=B)
     plan.host_sync()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    # the same, one call at a time (H2D, kernels, D2H serialised)
+    # the same, one call at a time (H2D, kernels, D2H serialised); the first call allocates the
+    # workspace and is not timed
+    stream = torch.cuda.current_stream()
+    plan.execute_host(h_ins[0], h_outs[0], nr_beams=B, stream=stream)
     t0 = time.perf_counter()
-    for i in range(2):
+    for i in range(3):
         plan.execute_host(h_ins[0], h_outs[0], nr_beams=B, stream=stream)
-    e2e_serial_s = (time.perf_counter() - t0) / 2
+    e2e_serial_s = (time.perf_counter() - t0) / 3
     h_in, h_out = h_ins[0], h_outs[0]
     e2e_s = max_over_ranks(e2e_s, world)
-
     adds = B * D * C * S
-    value = aggregate_value(adds, world, ms_step * 1e-3)
-    secs = S / s.sample_rate
-    rt = secs / (ms_step * 1e-3 / B)
+    e2e = {"value": aggregate_value(adds, world, e2e_s), "unit": UNIT,
+           "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
+           "d2h_bytes_per_step": h_out.numel() * h_out.element_size(),
+           "ms_per_step": e2e_s * 1e3, "ms_per_step_unpipelined": e2e_serial_s * 1e3,
+           "api": "dedisp_execute_host_async + dedisp_host_sync, %d pinned buffer sets" % nslot}
+    del h_ins, h_outs, h_in, h_out
+    case.close()
+    torch.cuda.empty_cache()
+
+    # ---- the other BASELINE.json configs, same event protocol (north star: per-config real-time
+    # factor and beams in real time); fewer steps for the long ones
+    others = {}
+    if not args.only and args.variant is None:
+        for name in wl.CONFIGS:
+            if name == s.name:
+                continue
+            o = wl.CONFIGS[name]
+            c = Case(o, rank, tune=args.tune)
+            ksteps = args.steps if o.nr_beams == 1 else max(3, args.steps // 4)
+            t_ms, p = time_device(c, ksteps, 3, barrier)
+            t_ms = max_over_ranks(t_ms, world)
+            others[name] = report(c, world, t_ms, p, ksteps, hbm_gbs, sm_max_mhz, peak_kind)
+            others[name]["steps"] = ksteps
+            c.close()
+            torch.cuda.empty_cache()
+
     if rank == 0:
-        kern_ms = float(np.mean(per))
-        comp = compulsory_bytes(s, in_samples)
         clk = (clocks or {}).get("sm_mhz") or sm_max_mhz
-        alu_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12  # T adds/s at max clock
-        achieved = adds / (kern_ms * 1e-3) / 1e12
+        head["roofline"]["note"] += "; frac at the observed clock (%.0f MHz): %.3f" % (
+            clk, head["roofline"]["frac"] * sm_max_mhz / clk)
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": dtype_name(s), "data": "synthetic",
-            "config": {"workload": workload_name(s), "variant": vname, "tuning": tuned,
-                       "l2": "rotating %d input/output buffer sets (%.0f MB) > 126 MB L2"
-                             % (nbuf, nbuf * set_bytes / 1e6),
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic",
+            "config": {"workload": head["workload"], "variant": head["variant"], "tuning": head["tuning"],
+                       "l2": head["l2"],
                        "replicas": "N independent replicas, no collective" if world > 1 else "1"},
-            "real_time_factor": rt, "beams_in_real_time": int(np.floor(rt)),
-            "beams_memory_cap": int(180e9 // (set_bytes / B)),
-            "ms_per_step_median": float(np.median(per)), "ms_per_step_min": float(per[0]),
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
-                         "frac": achieved / alu_peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(s.name),
-                         "note": "fp32/u32 adds per second vs 148 SMs x 128 lanes x %.0f MHz max SM "
-                                 "clock; frac at the observed clock (%.0f MHz): %.3f"
-                                 % (sm_max_mhz, clk, achieved / (SM_COUNT * FP32_LANES_PER_SM * clk * 1e6 / 1e12))},
-            "hbm_roofline": {"compulsory_bytes": comp, "achieved_gbs": comp / (kern_ms * 1e-3) / 1e9,
-                             "peak_gbs": hbm_gbs, "peak_kind": peak_kind,
-                             "frac": comp / (kern_ms * 1e-3) / 1e9 / hbm_gbs,
-                             "frac_of_nominal_8TBs": comp / (kern_ms * 1e-3) / 8e12},
-            "e2e": {"value": aggregate_value(adds, world, e2e_s), "unit": UNIT,
-                    "h2d_bytes_per_step": h_in.numel() * h_in.element_size(),
-                    "d2h_bytes_per_step": h_out.numel() * h_out.element_size(),
-                    "ms_per_step": e2e_s * 1e3, "ms_per_step_unpipelined": e2e_serial_s * 1e3,
-                    "api": "dedisp_execute_host_async + dedisp_host_sync, %d pinned buffer sets" % nslot},
-            "gpu_launches": args.steps * ((B + 65534) // 65535),
-            "clocks": clocks,
+            "real_time_factor": head["real_time_factor"], "beams_in_real_time": head["beams_in_real_time"],
+            "beams_memory_cap": head["beams_memory_cap"],
+            "ms_per_step_median": head["ms_per_step_median"], "ms_per_step_min": head["ms_per_step_min"],
+            "roofline": head["roofline"], "hbm_roofline": head["hbm_roofline"],
+            "e2e": e2e, "gpu_launches": head["gpu_launches"], "clocks": clocks,
         }
+        if others:
+            line["configs"] = others
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"], _ = cpu_baseline(s)
+            line["cpu_baseline"] = cpu_baseline(s)
         print(json.dumps(line))
-    plan.destroy()
     if world > 1:
         dist.destroy_process_group()
 
@@ -360,7 +472,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="apertif", choices=sorted(wl.CONFIGS))
-    ap.add_argument("--variant", type=int, default=None, help="force a kernel variant index")
+    ap.add_argument("--only", action="store_true", help="time the named config only")
+    ap.add_argument("--variant", type=int, default=None, help="force a kernel variant index (implies --only)")
     ap.add_argument("--tune", action="store_true", help="run dedisp_tune before timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -54,3 +54,13 @@ def test_single_rank_is_identity():
     import bench
     assert bench.max_over_ranks(3.5, 1) == 3.5
     assert bench.aggregate_value(2 * 10**9, 1, 1.0) == 2.0
+
+
+def test_gpus_flag_must_agree_with_the_launcher():
+    """`python bench.py --gpus 8` without torchrun would silently time one GPU: refused."""
+    sys.path.insert(0, ROOT)
+    import bench
+    bench.check_world(1, 1)
+    bench.check_world(4, 4)
+    with pytest.raises(SystemExit):
+        bench.check_world(8, 1)
