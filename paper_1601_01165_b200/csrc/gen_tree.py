@@ -30,72 +30,86 @@ def wn(dt: int, tt: int, q: int) -> int:
     return (3 + (dt - 1) * (q + 1) + tt + 3) // 4 * 4
 
 
-CTYPE = {"f32": ("float", "float4"), "u32": ("uint32_t", "uint4")}
+CTYPE = {"f32": ("float", "f32", "f"), "u32": ("uint32_t", "u32", "r")}
+
+# Descriptor word of one (channel, DM group), built by desc_kernel (shift_table.cu):
+#   [15:4] index of the 16-byte quad of the staged row the group's window starts in, so that
+#          d & 0xfff0 is the window's byte offset;  [1:0] m0, the first DM's offset inside that quad;
+#   [23:16] one-hot slope class, 0x10000 << q_c;  [31:24] bits, the group's increments being q_c + bit_j.
+# A descriptor with no slope bit (0) ends the chunk: the row after a chunk's last channel holds zeros.
+Q_SHIFT, BIT_SHIFT, OFF_MASK = 16, 24, 0xfff0
 
 
 def emit(dt: int, tt: int, qmax: int, typ: str = "f32") -> str:
     o = []
     wnmax = wn(dt, tt, qmax)
-    ct, vt = CTYPE[typ]
+    ct, pt, rc = CTYPE[typ]
     # u32: two warp-uniform run-time constants (0 and 1) that pin the pipe of each add, see tree_add
     xdecl = ", uint32_t zero, uint32_t one" if typ == "u32" else ""
     xargs = ", zero, one" if typ == "u32" else ""
     o.append("template <> struct TreeStep<%s, %d, %d, %d> {" % (ct, dt, tt, qmax))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
-    # one lattice per slope class q
+    # One function per slope class q: the channel loop over a run of channels of that class.  The loop
+    # has no head block.  Every node of the last DM ends with the loop's step: advance to the next
+    # channel, leave if its slope class differs (or it is the chunk's terminator), fetch the descriptor
+    # after it, issue the next channel's window loads, and branch on m0 straight to that channel's first
+    # node.  So the window loads are in flight while the branches resolve, and a channel costs about
+    # three taken branches instead of five.
     for q in range(qmax + 1):
         n = wn(dt, tt, q)
-        o.append("    // slope class q = %d.  p: 16-byte aligned window start in shared memory; m0, bits: "
-                 "warp-uniform" % q)
-        o.append("    static __device__ __forceinline__ void run_q%d(%s (&acc)[%d][%d], const %s *p, "
-                 "unsigned m0, unsigned bits%s) {" % (q, ct, dt, tt, ct, xdecl))
-        o.append("        %s w[%d];" % (ct, n))
-        o.append("        %s v;" % vt)
-        o.append("        const %s *p4 = reinterpret_cast<const %s *>(p);" % (vt, vt))
+        qbit = 1 << (Q_SHIFT + q)
+        loads = []
         for m in range(n // 4):
-            o.append("        v = p4[%d]; w[%d] = v.x; w[%d] = v.y; w[%d] = v.z; w[%d] = v.w;"
-                     % (m, 4 * m, 4 * m + 1, 4 * m + 2, 4 * m + 3))
-        o.append("        if (m0 & 2u) { if (m0 & 1u) goto N_0_3; else goto N_0_2; }")
-        o.append("        else { if (m0 & 1u) goto N_0_1; else goto N_0_0; }")
+            loads.append('asm volatile("ld.shared.v4.%s {%%0, %%1, %%2, %%3}, [%%4 + %d];" : "=%s"(w[%d]), '
+                         '"=%s"(w[%d]), "=%s"(w[%d]), "=%s"(w[%d]) : "r"(p));'
+                         % (pt, 16 * m, rc, 4 * m, rc, 4 * m + 1, rc, 4 * m + 2, rc, 4 * m + 3))
+        enter = ["dn = tree_desc<WD * 4>(ds);", "ds += WD * 4;", "p = rows + (d & %du);" % OFF_MASK] + loads + [
+            "if (d & 2u) { if (d & 1u) goto N_0_3; else goto N_0_2; }",
+            "else { if (d & 1u) goto N_0_1; else goto N_0_0; }"]
+        o.append("    // slope class q = %d: window of %d registers.  rows, ds: shared-memory byte addresses of the"
+                 % (q, n))
+        o.append("    // thread's place in the current channel's staged row and of the warp's descriptor of that")
+        o.append("    // channel; d: that descriptor (warp-uniform).  Returns at the first channel of another class.")
+        o.append("    template <int WD>")
+        o.append("    static __device__ __forceinline__ void loop_q%d(%s (&acc)[%d][%d], uint32_t &rows, "
+                 "uint32_t &ds, uint32_t &d, uint32_t lrow_b%s) {" % (q, ct, dt, tt, xdecl))
+        o.append("        %s w[%d];" % (ct, n))
+        o.append("        uint32_t dn, p;")
+        for line in enter:
+            o.append("        " + line)
         for j in range(dt):
             for r in range(j * q, j * q + 3 + j + 1):
                 o.append("    N_%d_%d:" % (j, r))
                 o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
                 if j + 1 < dt:
-                    o.append("        if (bits & %du) goto N_%d_%d; else goto N_%d_%d;"
-                             % (1 << j, j + 1, r + q + 1, j + 1, r + q))
+                    o.append("        if (d & %du) goto N_%d_%d; else goto N_%d_%d;"
+                             % (1 << (BIT_SHIFT + j), j + 1, r + q + 1, j + 1, r + q))
                 else:
-                    o.append("        goto DONE;")
-        o.append("    DONE:;")
+                    # the loop step, one copy per last node (the comment keeps the copies from being
+                    # merged back into one shared block behind a jump)
+                    o.append('        asm volatile("// step q%d r%d");' % (q, r))
+                    o.append("        rows += lrow_b;")
+                    o.append("        d = dn;")
+                    o.append("        if (!(d & %du)) goto OUT;" % qbit)
+                    for line in enter:
+                        o.append("        " + line)
+        o.append("    OUT:;")
         o.append("    }")
-    # the channel loop of one staged chunk.  The slope class is tested only when it changes: channels
-    # are ordered by frequency, so q_c is constant over long runs.  Testing single bits of a one-hot
-    # mask keeps the dispatch compare-and-branch (a chain of q == k tests with five or more cases is
-    # turned into an indirect jump through a constant-memory table, LDC + BRX).
-    o.append("    // rows: the thread's position in channel 0's staged row; ds: the warp's descriptor of")
-    o.append("    // channel 0, WD words per channel; the descriptor of the next channel is fetched one channel")
-    o.append("    // ahead (after the last channel this reads one row past the chunk: in bounds, never used)")
+    # the channel loop of one staged chunk.  Testing single bits of a one-hot mask keeps the dispatch
+    # compare-and-branch (a chain of q == k tests with five or more cases is turned into an indirect jump
+    # through a constant-memory table, LDC + BRX).  No channel counter: the zero descriptor after the
+    # chunk's last channel fails every slope test.
+    o.append("    // rows: shared-memory byte address of the thread's position in channel 0's staged row;")
+    o.append("    // ds: shared-memory byte address of the warp's descriptor of channel 0 (WD words per channel,")
+    o.append("    // a zero row after the last channel); lrow_b: bytes per staged row.")
     o.append("    template <int WD>")
-    o.append("    static __device__ __forceinline__ void chunk(%s (&acc)[%d][%d], const %s *rows, "
-             "const uint32_t *ds, int ncc, int lrow%s) {" % (ct, dt, tt, ct, xdecl))
-    o.append("        const uint32_t *const ds_end = ds + ncc * WD;")
-    o.append("        uint32_t d = tree_desc(ds), dn;")
+    o.append("    static __device__ __forceinline__ void chunk(%s (&acc)[%d][%d], uint32_t rows, "
+             "uint32_t ds, uint32_t lrow_b%s) {" % (ct, dt, tt, xdecl))
+    o.append("        uint32_t d = tree_desc<0>(ds);")
     o.append("    NEXT:")
-    for q in range(qmax):
-        o.append("        if (d & %du) goto L%d;" % (0x100 << q, q))
-    o.append("        goto L%d;" % qmax)
     for q in range(qmax + 1):
-        o.append("    L%d:" % q)
-        o.append("        do {")
-        o.append("            ds += WD;")
-        o.append("            dn = tree_desc(ds);")
-        o.append("            run_q%d(acc, rows + ((d >> 16) & ~3u), (d >> 16) & 3u, d & 0xffu%s);" % (q, xargs))
-        o.append("            rows += lrow;")
-        o.append("            d = dn;")
-        o.append("        } while (ds != ds_end && (d & %du));" % (0x100 << q))
-        o.append("        if (ds != ds_end) goto NEXT;")
-        o.append("        goto END;")
-    o.append("    END:;")
+        o.append("        if (d & %du) { loop_q%d<WD>(acc, rows, ds, d, lrow_b%s); goto NEXT; }"
+                 % (1 << (Q_SHIFT + q), q, xargs))
     o.append("    }")
     o.append("};")
     return "\n".join(o)
@@ -106,12 +120,12 @@ HEADER = """// GENERATED by gen_tree.py -- do not edit.  KIND_TREE add lattices 
 #include <stdint.h>
 namespace dedisp {
 template <typename E, int DT, int TT, int QMAX> struct TreeStep;
-// descriptor of one (channel, DM group): a shared-memory load whose address is the same for the whole
-// warp.  Explicit ld.shared keeps it out of the generic address space, whose loads the compiler's
-// divergence analysis treats as divergent.
-__device__ __forceinline__ uint32_t tree_desc(const uint32_t *p) {
+// descriptor of one (channel, DM group): a shared-memory load whose address (a 32-bit shared-window
+// byte address plus a constant) is the same for the whole warp.
+template <int OFF>
+__device__ __forceinline__ uint32_t tree_desc(uint32_t p) {
     uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)));
+    asm volatile("ld.shared.u32 %0, [%1 + %2];" : "=r"(v) : "r"(p), "n"(OFF));
     return v;
 }
 // acc[k] += w[R + k], all indices static.  Inline asm keeps the optimiser from merging the add

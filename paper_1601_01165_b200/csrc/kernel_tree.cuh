@@ -18,10 +18,12 @@
 //                integer add accumulates two outputs (t and t + S2) whatever the shift, odd or even;
 //                a CTA covers outputs [T0, T0 + HALF) and [S2 + T0, S2 + T0 + HALF).  The counters
 //                are flushed into the uint32 output every <= 256 channels (256 * 255 < 2^16).
-//   per channel: one descriptor word per (channel, DM group) built at plan creation
-//                (desc_kernel, shift_table.cu):  [31:16] window offset in the staged row
-//                [15:8] 1 << q_c   [7:0] bits, the group's shift increments being q_c + bit_j.
-//                Staged per chunk next to the input rows.
+//   per channel: one descriptor word per (channel, DM group), built when the variant is selected
+//                (desc_kernel, shift_table.cu; layout in gen_tree.py): the window's byte offset in
+//                the staged row, the first DM's offset in its 16-byte quad, the channel's slope
+//                class q_c one-hot, and the bits b_j, the group's shift increments being q_c + b_j.
+//                Staged per chunk next to the rows; the row after the chunk's last channel is zero
+//                and ends the channel loop.
 #pragma once
 #include <type_traits>
 
@@ -56,11 +58,11 @@ struct TreeTile {
     static_assert(HALF % AL == 0, "time tiles start on 16-byte boundaries of the staged rows");
 };
 
-// Shared memory (dynamic): mbarriers | NSTAGE stages { CC rows of lrow staged elements | CC x WD
-// descriptors }.
+// Shared memory (dynamic): mbarriers | NSTAGE stages { CC rows of lrow staged elements | (CC + 1) x WD
+// descriptors, the last row a terminator }.
 template <typename T>
 __host__ __device__ inline size_t tree_stage_bytes(int lrow) {
-    return (size_t)T::CC * ((size_t)lrow * 4 + (size_t)T::WD * 4);
+    return (size_t)T::CC * ((size_t)lrow * 4 + (size_t)T::WD * 4) + (size_t)T::WD * 4;
 }
 template <typename T>
 __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
@@ -78,6 +80,10 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const typename T::Stg
     const int s = k % T::NSTAGE;
     const int c = k * T::CC + lane;
     uint32_t bytes = 0;
+    // ragged last chunk: the descriptor row after its last channel ends the channel loop
+    const int ncc = a.C - k * T::CC;
+    if (ncc < T::CC && lane < T::WD)
+        reinterpret_cast<uint32_t *>(stages + (size_t)s * sbytes + data_bytes)[ncc * T::WD + lane] = 0u;
     if (lane < T::CC && c < a.C) {
         const int32_t *trow = a.shiftT + (size_t)c * a.dpitch + dm_lo;
         const int smin = trow[0], smax = trow[T::DMS_CTA - 1];
@@ -96,6 +102,7 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const typename T::Stg
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+    __syncwarp();  // the terminator row is written before lane 0's (releasing) arrive
     if (lane == 0) mbar_arrive_expect_tx(&full[s], bytes);
 }
 
@@ -132,6 +139,10 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
         }
         mbar_fence_init();
     }
+    // the terminator descriptor row of every stage (row CC; never overwritten by the copies)
+    if (threadIdx.x < T::NSTAGE * T::WD)
+        reinterpret_cast<uint32_t *>(stages + (size_t)(threadIdx.x / T::WD) * sbytes + data_bytes)
+            [T::CC * T::WD + threadIdx.x % T::WD] = 0u;
     __syncthreads();
     // prologue: warp 0 fills the first NSTAGE-1 stages
     constexpr int AHEAD = T::NSTAGE - 1;
@@ -210,18 +221,26 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     const int phase = T::U8 ? (warp * T::FLUSH_CHUNKS) / T::NW : 0;
     bool flushed = false;
 
+    // Loop constants pinned in registers (an opaque move: otherwise they are re-read from the constant
+    // bank and moved into a register in every channel of the loop below).
+    uint32_t lrow_b, zero, one;
+    asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
+    asm volatile("mov.u32 %0, %1;" : "=r"(zero) : "r"(a.zero));
+    asm volatile("mov.u32 %0, %1;" : "=r"(one) : "r"(a.one));
+    const uint32_t stages_s = smem_u32(stages);
+    const uint32_t my_row = (uint32_t)(tw + lane * T::TT) * 4;      // the thread's place in a row
+    const uint32_t my_desc = (uint32_t)data_bytes + (uint32_t)g * 4;  // the warp's descriptor column
+
     for (int k = 0; k < nchunks; ++k) {
         const int s = k % T::NSTAGE;
-        const int ncc = (a.C - k * T::CC) < T::CC ? (a.C - k * T::CC) : T::CC;
         mbar_wait(&full[s], (k / T::NSTAGE) & 1);
-        const unsigned char *st = stages + (size_t)s * sbytes;
-        const Elem *rows = reinterpret_cast<const Elem *>(st) + tw + lane * T::TT;
-        const uint32_t *ds = reinterpret_cast<const uint32_t *>(st + data_bytes) + g;
+        const uint32_t st = stages_s + (uint32_t)s * (uint32_t)sbytes;
         if constexpr (T::U8)
-            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, rows, ds, ncc, a.lrow,
-                                                                         a.zero, a.one);
+            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
+                                                                         lrow_b, zero, one);
         else
-            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, rows, ds, ncc, a.lrow);
+            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
+                                                                         lrow_b);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
         // producer duty, rotating over the warps (step a4): refill the most recently released

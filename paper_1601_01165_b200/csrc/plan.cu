@@ -118,7 +118,7 @@ static int ensure_tree_table(dedisp_plan *pl, int v) {
         return DEDISP_ERR_CUDA;
     }
     cudaFree(d_flags);
-    if (h[1] != 0) {  // a window offset past 16 bits: tree_fit excludes such plans
+    if (h[1] != 0) {  // a window offset past 14 bits: tree_fit excludes such plans
         cudaFree(t.d_desc);
         return DEDISP_ERR_INVALID_ARG;
     }

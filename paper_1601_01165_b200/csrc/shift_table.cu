@@ -90,13 +90,14 @@ __global__ void chan_slope_kernel(const int32_t *shiftT, int D, int dpitch, int 
 }
 
 // desc_kernel: one thread per (channel c, DM group G of dt DMs); the group belongs to the CTA tile
-// of dms_cta DMs that starts at DM lo = (G*dt / dms_cta) * dms_cta.
-//   desc[c][G] = woff << 16 | (1 << q_c) << 8 | bits          (dt <= 9, q_c <= 7)
+// of dms_cta DMs that starts at DM lo = (G*dt / dms_cta) * dms_cta.  With
 //   woff = shift(c, G*dt) - (shift(c, lo) & ~(al-1)): offset of the group's first DM in the staged
-//          row, whose element 0 is input sample T0 + (shift(c, lo) & ~(al-1));
-//   bits: increment j of the group = q_c + bit (j-1).
+//          row, whose element 0 is row element T0 + (shift(c, lo) & ~(al-1)),
+//   desc[c][G] = bits << 24 | (0x10000 << q_c) | (woff >> 2) << 4 | (woff & 3)      (gen_tree.py)
+// i.e. d & 0xfff0 is the byte offset of the 16-byte quad the window starts in, d & 3 the first DM's
+// offset in it, and increment j of the group = q_c + bit (j-1)  (dt <= 9, q_c <= 7).
 // DMs past D (ragged last group, padding groups) continue with increment q_c: their outputs are
-// never stored and their window offsets stay inside the lattice.  flags[1] |= 1 if woff >= 2^16.
+// never stored and their window offsets stay inside the lattice.  flags[1] |= 1 if woff >= 2^14.
 __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, int dpitch, int dt,
                             int dms_cta, int al, int descpitch, uint32_t *desc, int *flags) {
     int G = blockIdx.x * blockDim.x + threadIdx.x;
@@ -106,7 +107,7 @@ __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, 
     const long d0 = (long)G * dt;
     const long lo = d0 / dms_cta * dms_cta;
     const int e0 = row[d0 < D ? d0 : D - 1];
-    const int base = row[lo < D ? lo : D - 1] & ~(al - 1);  // al = input elements per 16 bytes
+    const int base = row[lo < D ? lo : D - 1] & ~(al - 1);  // al = staged elements per 16 bytes
     const int q = qc[c];
     uint32_t bits = 0;
     for (int j = 1; j < dt && d0 + j < D; ++j) {
@@ -115,8 +116,9 @@ __global__ void desc_kernel(const int32_t *shiftT, const int *qc, int C, int D, 
         bits |= (uint32_t)b << (j - 1);
     }
     const int woff = e0 - base;
-    if (woff < 0 || woff > 0xffff) atomicOr(&flags[1], 1);
-    desc[(size_t)c * descpitch + G] = ((uint32_t)woff & 0xffffu) << 16 | (0x100u << q) | bits;
+    if (woff < 0 || woff > 0x3fff) atomicOr(&flags[1], 1);
+    const uint32_t w = (uint32_t)woff & 0x3fffu;
+    desc[(size_t)c * descpitch + G] = bits << 24 | (0x10000u << q) | (w >> 2) << 4 | (w & 3u);
 }
 
 // pack_pairs_kernel: the uint8 tree kernels' view of the input (kernel_tree.cuh).  One thread per four

@@ -117,7 +117,7 @@ VariantFit tree_fit(const Variant &v, const PlanShape &p, int span_cta) {
     // window over-read past the last offset a descriptor can hold
     long lrow = (long)T::HALF + span_cta + 2 * T::AL + T::WNMAX;
     lrow = (lrow + T::AL - 1) / T::AL * T::AL;
-    if (span_cta + T::AL > 0xffff) return f;  // window offsets are 16-bit descriptor fields
+    if (span_cta + T::AL > 0x3fff) return f;  // window offsets are 14-bit descriptor fields
     size_t smem = tree_smem_bytes<T>((int)lrow);
     if (smem > kMaxSmem) return f;
     const long span_t = T::U8 ? p.S2 : p.S;  // elements along time the grid has to cover
