@@ -39,9 +39,9 @@ INT_LANES_PER_SM = 128           # 32-bit integer adds: 64 lanes on the integer 
 LDS_WORDS_PER_SM = 32            # shared memory: 128 bytes per clock and SM
 FALLBACK_HBM_GBS = 6650.0        # B200_PROFILING.md fallback
 FALLBACK_SM_MHZ = 1965.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full captures summarised
-# under profiles/ (the JSON names the file each number comes from)
-TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+# dram__bytes_read.sum + dram__bytes_write.sum per step, from the ncu --set full captures summarised
+# under profiles/ (the table names the file each number comes from; profiles/r02_traffic.md)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
 
 
 def measured_peaks():
@@ -57,13 +57,15 @@ def measured_peaks():
 
 def ncu_traffic(config_name, variant_name):
     """(bytes per step, source) for the config if profiles/ holds a capture of this variant."""
+    import csv
     try:
-        d = json.load(open(TRAFFIC_JSON))[config_name]
+        rows = {r["config"]: r for r in csv.DictReader(open(TRAFFIC_CSV))}
+        d = rows[config_name]
     except Exception:
         return None, None
-    if d.get("variant") and d["variant"] != variant_name:
+    if d["variant"] != variant_name:
         return None, "profiles capture is of another variant: " + d["variant"]
-    return d["dram_bytes_per_step"], d["source"]
+    return int(d["dram_bytes_per_step"]), d["source"]
 
 
 def compulsory_bytes(s, in_samples):
