@@ -39,6 +39,12 @@ EDGES = [
     wl.Setup("beams3_u8", 20, 1400.0, 3.0, 20000.0, 900, 0.0, 0.25, 50, nr_beams=3, in_dtype=wl.U8, values="u8", seed=11),
     wl.Setup("big_steps", 16, 140.0, 0.2, 100000.0, 3000, 0.0, 0.05, 40, seed=12),    # LOFAR-like long shifts
     wl.Setup("dm_first_nonzero", 32, 1420.0, 1.0, 20000.0, 1500, 100.0, 0.25, 45, seed=13),
+    # uint8 pair layout: S/2 not a multiple of 4, fewer samples than one pair quad, one DM, and more than
+    # 512 channels (three counter flushes) on ragged tiles
+    wl.Setup("u8_one_sample", 9, 1400.0, 3.0, 20000.0, 1, 0.0, 0.25, 3, in_dtype=wl.U8, values="u8", seed=14),
+    wl.Setup("u8_s6", 20, 1400.0, 3.0, 20000.0, 6, 0.0, 0.25, 21, in_dtype=wl.U8, values="u8", seed=15),
+    wl.Setup("u8_one_dm", 40, 1400.0, 2.0, 10000.0, 1303, 3.0, 0.0, 1, in_dtype=wl.U8, values="u8", seed=16),
+    wl.Setup("u8_flush3", 700, 1220.0, 300.0 / 700, 24414.0, 1502, 0.0, 0.2, 37, in_dtype=wl.U8, values="u8", seed=17),
 ]
 
 
