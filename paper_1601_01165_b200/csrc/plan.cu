@@ -140,9 +140,31 @@ static int prepare_variant(dedisp_plan *pl, int v) {
     return ensure_tree_table(pl, v);
 }
 
+// Adds per clock and SM the tree tiles sustain on B200 (round-2 measurements on apertif / survey8, tile
+// and wave quantisation divided out): {uint8?, DT, samples per thread and DM, warps per CTA, rate}.
+// Tiles not listed fall back to a formula.  Only the untuned default uses this; dedisp_tune measures.
+static double tree_rate(bool u8, int dt, int tt, int warps, int cc) {
+    static const struct { int u8, dt, tt, warps; double rate; } kRates[] = {
+        {0, 4, 28, 12, 76}, {0, 5, 20, 12, 74}, {0, 6, 28, 8, 71}, {0, 6, 12, 16, 68}, {0, 4, 20, 12, 66},
+        {0, 4, 44, 8, 65},  {0, 5, 12, 16, 63}, {0, 5, 36, 8, 63}, {0, 8, 20, 8, 62},  {0, 6, 12, 12, 60},
+        {0, 4, 28, 8, 60},  {0, 4, 12, 16, 60}, {0, 6, 20, 8, 57}, {0, 8, 12, 12, 57}, {0, 4, 36, 8, 62},
+        {1, 5, 24, 16, 108}, {1, 4, 40, 12, 107}, {1, 5, 40, 12, 100}, {1, 4, 24, 16, 101}, {1, 6, 24, 12, 87},
+        {1, 6, 24, 16, 84},  {1, 4, 56, 12, 92},  {1, 8, 24, 12, 79},  {1, 4, 72, 8, 82},   {1, 6, 56, 8, 64},
+        {1, 8, 40, 8, 47},
+    };
+    double rate = -1;
+    for (const auto &r : kRates)
+        if (r.u8 == (int)u8 && r.dt == dt && r.tt == tt && r.warps == warps) rate = r.rate;
+    if (rate < 0) {
+        const double tile = (double)dt * tt;
+        rate = (tile >= 100 ? (warps >= 12 ? 62 : 58) : tile >= 72 ? 52 : 42) * (u8 ? 1.4 : 1.0);
+    }
+    return rate * (cc >= 12 ? 1.0 : 0.93);  // 8-channel stages: more chunk bookkeeping per add
+}
+
 // Untuned default: a cost model in SM clocks.  A CTA costs the larger of its adds at the kind's
 // measured rate (adds/clk/SM on B200: tree ~58 for large thread tiles, lds ~28 = the one-word-per-add
-// shared-memory cap, generic ~10 = 4-byte loads at the L2's per-SM share) and of the bytes it stages
+// shared-memory cap, generic ~10 = 4-byte loads at the L2's per-SM share; tree tiles: tree_rate) and of the bytes it stages
 // from L2 (~40 B/clk/SM); an SM runs ceil(CTAs / 148) of them (wave quantisation), more slowly when
 // too few warps are resident to hide latencies.  dedisp_tune replaces the guess by a measurement.
 static int heuristic_variant(const dedisp_plan *pl) {
@@ -156,12 +178,11 @@ static int heuristic_variant(const dedisp_plan *pl) {
         const double tile = (double)x.dt * x.tt;
         double rate, need, occ;
         if (x.kind == KIND_TREE) {
-            rate = (tile >= 100 ? (x.threads >= 384 ? 62 : 58) : tile >= 72 ? 52 : 42) *
-                   (pl->dtype == DEDISP_U8 ? 1.4 : 1.0);  // uint8: two adds per integer add
+            rate = tree_rate(pl->dtype == DEDISP_U8, x.dt, x.tt, x.threads / 32, x.cc);
             need = 8;
             occ = x.threads <= 128 ? 4 : (x.threads <= 256 && tile <= 48) ? 2 : 1;
         } else if (x.kind == KIND_LDS) {
-            rate = tile >= 32 ? 28 : tile >= 16 ? 24 : 14;
+            rate = (x.dt == 4 && x.tt == 16) ? 30 : tile >= 32 ? 28 : tile >= 16 ? 24 : 14;
             need = 16;
             occ = std::floor(227.0 * 1024 / (double)std::max<size_t>(pl->fit[v].smem, 1));
             occ = std::max(1.0, std::min(occ, std::floor(2048.0 / x.threads)));
