@@ -78,6 +78,9 @@ TREE = [
     ("float", 8, 1, 5, 36, 8, 4, 3, 1),     # 40 x 1152
     ("float", 8, 1, 4, 44, 8, 3, 3, 1),     # 32 x 1408
     ("float", 8, 1, 4, 36, 16, 3, 3, 1),    # 32 x 1152
+    # ---- fp32, coarse DM grids: shifts growing by up to 7-8 samples per DM step (q <= 7)
+    ("float", 12, 1, 4, 20, 16, 3, 7, 1),   # 48 x 640
+    ("float", 12, 1, 4, 20, 8, 4, 7, 1),
     # ---- fp32, small problems (several CTAs per SM)
     ("float", 8, 1, 4, 12, 8, 3, 4, 2),     # 32 x 384, 2 CTAs/SM
     ("float", 4, 1, 4, 12, 8, 3, 4, 4),     # 16 x 384
@@ -102,6 +105,7 @@ TREE = [
     ("uint8_t", 8, 1, 8, 20, 8, 3, 4, 1),   # 64 x 1280
     ("uint8_t", 8, 1, 4, 36, 8, 3, 4, 1),   # 32 x 2304
     ("uint8_t", 12, 1, 8, 12, 8, 3, 4, 1),  # 96 x 768
+    ("uint8_t", 12, 1, 4, 20, 16, 3, 7, 1), # 48 x 1280, q <= 7 (coarse DM grids)
     ("uint8_t", 4, 1, 4, 12, 8, 3, 4, 4),   # 16 x 768, small problems
 ]
 

@@ -66,11 +66,22 @@ def test_slope_class_4_only_runs_q4_lattices(dd):
     assert q == 4 and n >= 3
 
 
+def test_slope_classes_up_to_7_run_the_coarse_grid_lattices(dd):
+    # Apertif band with a DM step of 0.5: shifts grow by up to 6.6 samples per step at the lowest channel
+    s = wl.scaled(wl.APERTIF, name="q6_f32", nr_channels=96, channel_bw_MHz=300.0 / 96, nr_dms=101,
+                  nr_samples=2700, dm_step=0.5, values="int16")
+    n, q = run_tree(dd, s, exact=True)
+    assert q == 6 and n >= 2
+    s8 = wl.scaled(s, name="q6_u8", in_dtype=wl.U8, values="u8")
+    n, q = run_tree(dd, s8, exact=True)
+    assert q == 6 and n >= 1
+
+
 def test_slope_beyond_the_lattice_falls_back_to_other_kinds(dd):
     s = wl.scaled(wl.SURVEY8, name="q9", nr_channels=64, channel_bw_MHz=300.0 / 64, nr_dms=40,
                   nr_samples=1500, dm_step=0.5, in_dtype=wl.F32, values="int16")
     with dd.Plan(*s.plan_args()) as plan:
-        assert max_q(oracle.shift_table(*s.table_args())) > 4
+        assert max_q(oracle.shift_table(*s.table_args())) > 7
         assert not tree_variants(dd, plan)
         assert plan.supported_variants()  # lds / generic still run it
 
