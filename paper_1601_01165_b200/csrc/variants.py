@@ -64,6 +64,10 @@ TREE = [
     ("float", 16, 1, 6, 12, 16, 3, 4, 1),
     ("float", 16, 1, 4, 12, 16, 3, 4, 1),   # 64 x 384
     ("float", 16, 1, 5, 12, 16, 3, 3, 1),   # 80 x 384
+    ("float", 16, 1, 4, 20, 16, 3, 3, 1),   # 64 x 640
+    ("float", 16, 1, 4, 20, 12, 4, 3, 1),
+    ("float", 16, 1, 4, 20, 20, 3, 3, 1),
+    ("float", 16, 1, 4, 20, 8, 4, 3, 1),
     # ---- fp32, 8 warps/SM (<= 255 registers)
     ("float", 8, 1, 8, 20, 8, 4, 3, 1),     # 64 x 640
     ("float", 8, 1, 8, 20, 8, 4, 4, 1),
@@ -95,6 +99,14 @@ TREE = [
     ("uint8_t", 12, 1, 4, 28, 12, 3, 4, 1),
     ("uint8_t", 12, 1, 5, 20, 16, 3, 4, 1),
     ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1),
+    ("uint8_t", 16, 1, 5, 12, 12, 4, 4, 1),
+    ("uint8_t", 16, 1, 5, 12, 16, 4, 4, 1),
+    ("uint8_t", 16, 1, 5, 12, 24, 2, 4, 1),
+    ("uint8_t", 16, 1, 5, 12, 32, 2, 4, 1),
+    ("uint8_t", 16, 1, 4, 20, 16, 3, 4, 1),  # 64 x 1280, 16 warps
+    ("uint8_t", 16, 1, 4, 20, 12, 4, 4, 1),
+    ("uint8_t", 16, 1, 4, 20, 24, 2, 4, 1),
+    ("uint8_t", 16, 1, 4, 20, 12, 3, 4, 1),
     ("uint8_t", 16, 1, 4, 12, 16, 3, 4, 1),
     ("uint8_t", 12, 1, 5, 20, 8, 3, 4, 1),  # 60 x 1280
     ("uint8_t", 12, 1, 6, 12, 8, 3, 4, 1),  # 72 x 768
