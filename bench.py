@@ -432,13 +432,21 @@ def run_ours(args, s):
             if name == s.name:
                 continue
             o = wl.CONFIGS[name]
-            c = Case(o, rank, tune=args.tune)
-            ksteps = args.steps if o.nr_beams == 1 else max(3, args.steps // 4)
-            t_ms, p = time_device(c, ksteps, 3, barrier)
-            t_ms = max_over_ranks(t_ms, world)
-            others[name] = report(c, world, t_ms, p, ksteps, hbm_gbs, sm_max_mhz, peak_kind)
-            others[name]["steps"] = ksteps
-            c.close()
+            # a config that cannot run here (e.g. batch40's 11 GB on a smaller device) is reported as
+            # such; the headline line is printed either way (single rank only: with replicas every
+            # rank must reach the same collectives)
+            try:
+                c = Case(o, rank, tune=args.tune)
+                ksteps = args.steps if o.nr_beams == 1 else max(3, args.steps // 4)
+                t_ms, p = time_device(c, ksteps, 3, barrier)
+                t_ms = max_over_ranks(t_ms, world)
+                others[name] = report(c, world, t_ms, p, ksteps, hbm_gbs, sm_max_mhz, peak_kind)
+                others[name]["steps"] = ksteps
+                c.close()
+            except Exception as e:  # noqa: BLE001
+                if world > 1:
+                    raise
+                others[name] = {"workload": workload_name(o), "error": "%s: %s" % (type(e).__name__, e)}
             torch.cuda.empty_cache()
 
     if rank == 0:
