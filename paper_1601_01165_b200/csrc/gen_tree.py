@@ -18,10 +18,11 @@ Two element types: "f32" (fp32 input: float accumulators, FADD / packed FADD2) a
 staged as pairs of 16-bit counters in one 32-bit word, kernel_tree.cuh: one integer add does two adds
 whatever the offset).
 
-Usage: python gen_tree.py OUT.cuh TYPE:DT,TT,QMAX [TYPE:DT,TT,QMAX ...]
+Usage: python gen_tree.py OUTDIR TYPE:DT,TT,QMAX,LAZY [TYPE:DT,TT,QMAX,LAZY ...]
 """
 from __future__ import annotations
 
+import os
 import sys
 
 
@@ -40,14 +41,26 @@ CTYPE = {"f32": ("float", "f32", "f"), "u32": ("uint32_t", "u32", "r")}
 Q_SHIFT, BIT_SHIFT, OFF_MASK = 16, 24, 0xfff0
 
 
-def emit(dt: int, tt: int, qmax: int, typ: str = "f32") -> str:
+def need(r: int, tt: int) -> int:
+    """Highest 16-byte quad of the window a DM at offset r reads (w[r .. r+tt))."""
+    return (r + tt - 1) // 4
+
+
+def first_lazy(tt: int, q: int) -> int:
+    """LAZY lattices: quads below this index are loaded when a channel starts, the others only on the
+    paths that read them.  No first or second DM of a group ever reads a lazy quad (their offsets are at
+    most 3 and 4 + q), so a lazy quad is always requested at least one add block ahead of its use."""
+    return need(4 + q, tt) + 1
+
+
+def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
     o = []
     wnmax = wn(dt, tt, qmax)
     ct, pt, rc = CTYPE[typ]
     # u32: two warp-uniform run-time constants (0 and 1) that pin the pipe of each add, see tree_add
     xdecl = ", uint32_t zero, uint32_t one" if typ == "u32" else ""
     xargs = ", zero, one" if typ == "u32" else ""
-    o.append("template <> struct TreeStep<%s, %d, %d, %d> {" % (ct, dt, tt, qmax))
+    o.append("template <> struct TreeStep<%s, %d, %d, %d, %d> {" % (ct, dt, tt, qmax, lazy))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
     # One function per slope class q: the channel loop over a run of channels of that class.  The loop
     # has no head block.  Every node of the last DM ends with the loop's step: advance to the next
@@ -55,19 +68,30 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32") -> str:
     # after it, issue the next channel's window loads, and branch on m0 straight to that channel's first
     # node.  So the window loads are in flight while the branches resolve, and a channel costs about
     # three taken branches instead of five.
+    #
+    # LAZY = 1: shared memory is what binds these kernels, and a quarter of the window words loaded up
+    # front are never read: the window is sized for the largest offset the last DM can reach
+    # (3 + (DT-1)(q+1)), the typical path stops short of it.  So only the quads below first_lazy() are
+    # loaded when the channel starts; node (j, R) requests the quads its successors read and the path so
+    # far has not: those both successors need at the node's start, the one only the bit = 1 successor
+    # needs on that edge.  Invariant: entering node (j, R), the quads loaded are exactly the up-front ones
+    # plus the lazy ones up to need(R); it depends on R alone, not on the path.
     for q in range(qmax + 1):
         n = wn(dt, tt, q)
         qbit = 1 << (Q_SHIFT + q)
+        nq = n // 4
+        upfront = min(nq, first_lazy(tt, q)) if lazy else nq
         loads = []
-        for m in range(n // 4):
+        for m in range(nq):
             loads.append('asm volatile("ld.shared.v4.%s {%%0, %%1, %%2, %%3}, [%%4 + %d];" : "=%s"(w[%d]), '
                          '"=%s"(w[%d]), "=%s"(w[%d]), "=%s"(w[%d]) : "r"(p));'
                          % (pt, 16 * m, rc, 4 * m, rc, 4 * m + 1, rc, 4 * m + 2, rc, 4 * m + 3))
-        enter = ["dn = tree_desc<WD * 4>(ds);", "ds += WD * 4;", "p = rows + (d & %du);" % OFF_MASK] + loads + [
+        enter = ["dn = tree_desc<WD * 4>(ds);", "ds += WD * 4;", "p = rows + (d & %du);" % OFF_MASK] + \
+            loads[:upfront] + [
             "if (d & 2u) { if (d & 1u) goto N_0_3; else goto N_0_2; }",
             "else { if (d & 1u) goto N_0_1; else goto N_0_0; }"]
-        o.append("    // slope class q = %d: window of %d registers.  rows, ds: shared-memory byte addresses of the"
-                 % (q, n))
+        o.append("    // slope class q = %d: window of %d registers%s.  rows, ds: shared-memory byte addresses of the"
+                 % (q, n, ", quads %d.. on demand" % upfront if upfront < nq else ""))
         o.append("    // thread's place in the current channel's staged row and of the warp's descriptor of that")
         o.append("    // channel; d: that descriptor (warp-uniform).  Returns at the first channel of another class.")
         o.append("    template <int WD>")
@@ -80,11 +104,22 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32") -> str:
         for j in range(dt):
             for r in range(j * q, j * q + 3 + j + 1):
                 o.append("    N_%d_%d:" % (j, r))
-                o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
                 if j + 1 < dt:
-                    o.append("        if (d & %du) goto N_%d_%d; else goto N_%d_%d;"
-                             % (1 << (BIT_SHIFT + j), j + 1, r + q + 1, j + 1, r + q))
+                    have = max(upfront - 1, need(r, tt))          # highest quad loaded on entry
+                    both = range(have + 1, need(r + q, tt) + 1)    # read by both successors
+                    edge = range(max(have, need(r + q, tt)) + 1, need(r + q + 1, tt) + 1)  # by bit = 1 only
+                    for m in both:
+                        o.append("        " + loads[m])
+                    o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
+                    if len(edge):
+                        o.append("        if (d & %du) { %s goto N_%d_%d; } else goto N_%d_%d;"
+                                 % (1 << (BIT_SHIFT + j), " ".join(loads[m] for m in edge), j + 1, r + q + 1,
+                                    j + 1, r + q))
+                    else:
+                        o.append("        if (d & %du) goto N_%d_%d; else goto N_%d_%d;"
+                                 % (1 << (BIT_SHIFT + j), j + 1, r + q + 1, j + 1, r + q))
                 else:
+                    o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
                     # the loop step, one copy per last node (the comment keeps the copies from being
                     # merged back into one shared block behind a jump)
                     o.append('        asm volatile("// step q%d r%d");' % (q, r))
@@ -119,7 +154,7 @@ HEADER = """// GENERATED by gen_tree.py -- do not edit.  KIND_TREE add lattices 
 #pragma once
 #include <stdint.h>
 namespace dedisp {
-template <typename E, int DT, int TT, int QMAX> struct TreeStep;
+template <typename E, int DT, int TT, int QMAX, int LAZY> struct TreeStep;
 // descriptor of one (channel, DM group): a shared-memory load whose address (a 32-bit shared-window
 // byte address plus a constant) is the same for the whole warp.
 template <int OFF>
@@ -171,22 +206,33 @@ __device__ __forceinline__ void tree_add(uint32_t (&acc)[TT], const uint32_t (&w
 """
 
 
-def main(argv):
-    out = argv[1]
-    combos = sorted({(a.split(":")[0],) + tuple(int(x) for x in a.split(":")[1].split(","))
-                     for a in argv[2:]})
-    parts = [HEADER]
-    for typ, dt, tt, qmax in combos:
-        parts.append(emit(dt, tt, qmax, typ))
-    parts.append("}  // namespace dedisp\n")
-    text = "\n".join(parts)
+def combo_file(typ, dt, tt, qmax, lazy):
+    return "tree_gen_%s_%d_%d_%d_%d.cuh" % (typ, dt, tt, qmax, lazy)
+
+
+def _write_if_changed(path, text):
     try:
-        if open(out).read() == text:
+        if open(path).read() == text:
             return
     except OSError:
         pass
-    with open(out, "w") as f:
+    with open(path, "w") as f:
         f.write(text)
+
+
+def main(argv):
+    """Writes OUTDIR/tree_gen_common.cuh and one OUTDIR/tree_gen_<combo>.cuh per lattice (a unit includes
+    only its own, so changing one lattice recompiles one unit).  Files whose text is unchanged keep their
+    timestamps."""
+    outdir = argv[1]
+    combos = sorted({(a.split(":")[0],) + tuple(int(x) for x in a.split(":")[1].split(","))
+                     for a in argv[2:]})
+    _write_if_changed(os.path.join(outdir, "tree_gen_common.cuh"), HEADER + "}  // namespace dedisp\n")
+    for typ, dt, tt, qmax, lazy in combos:
+        _write_if_changed(os.path.join(outdir, combo_file(typ, dt, tt, qmax, lazy)),
+                          "// GENERATED by gen_tree.py -- do not edit.\n#pragma once\n"
+                          '#include "tree_gen_common.cuh"\nnamespace dedisp {\n'
+                          + emit(dt, tt, qmax, typ, lazy) + "\n}  // namespace dedisp\n")
 
 
 if __name__ == "__main__":

@@ -28,12 +28,16 @@
 #include <type_traits>
 
 #include "kernels.cuh"
-#include "build/tree_gen.cuh"
+#ifdef DEDISP_TREE_GEN
+#include DEDISP_TREE_GEN          // the one lattice this translation unit instantiates (build.py)
+#else
+#include "build/tree_gen_common.cuh"
+#endif
 
 namespace dedisp {
 
 template <typename In_, int WD_, int WT_, int DT_, int TT_, int CC_, int NSTAGE_, int QMAX_,
-          int MINB_>
+          int MINB_, int LAZY_ = 0>
 struct TreeTile {
     typedef In_ In;                              // float or uint8_t
     typedef typename AccOf<In_>::type Acc;       // output type: float / uint32_t
@@ -44,13 +48,15 @@ struct TreeTile {
     static constexpr int AL = 4;                 // staged elements per 16 bytes
     static constexpr int WD = WD_, WT = WT_, DT = DT_, TT = TT_, CC = CC_, NSTAGE = NSTAGE_,
                          QMAX = QMAX_, MINB = MINB_;
+    // LAZY = 1: the upper window quads are loaded only on the lattice paths that read them (gen_tree.py)
+    static constexpr int LAZY = LAZY_;
     static constexpr int NW = WD * WT;
     static constexpr int THREADS = NW * 32;
     static constexpr int DMS_CTA = WD * DT;
     static constexpr int HALF = WT * 32 * TT;    // elements per CTA along time
     static constexpr int SAMPLES_CTA = U8 ? 2 * HALF : HALF;  // outputs per DM and CTA
     static constexpr int FLUSH_CHUNKS = 256 / CC;  // uint8: chunks between counter flushes
-    static constexpr int WNMAX = TreeStep<Elem, DT, TT, QMAX>::WNMAX;
+    static constexpr int WNMAX = TreeStep<Elem, DT, TT, QMAX, LAZY>::WNMAX;
     static_assert(TT % 4 == 0, "thread windows are loaded with LDS.128");
     static_assert(WD % 4 == 0, "descriptor rows are copied in 16-byte units");
     static_assert(CC <= 32, "one lane per channel of a chunk issues its copies");
@@ -236,10 +242,10 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
         mbar_wait(&full[s], (k / T::NSTAGE) & 1);
         const uint32_t st = stages_s + (uint32_t)s * (uint32_t)sbytes;
         if constexpr (T::U8)
-            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
+            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
                                                                          lrow_b, zero, one);
         else
-            TreeStep<Elem, T::DT, T::TT, T::QMAX>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
+            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
                                                                          lrow_b);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);

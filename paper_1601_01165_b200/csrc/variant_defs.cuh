@@ -146,9 +146,9 @@ template <typename T>
 Variant make_tree() {
     static char name[112];
     snprintf(name, sizeof name,
-             "tree_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d q%d b%d",
+             "tree_%s: %dx%d DMsxsamples/CTA, %dx%d outputs/thread, cc%d s%d q%d b%d%s",
              T::U8 ? "u8" : "f32", T::DMS_CTA, T::SAMPLES_CTA, T::DT, T::U8 ? 2 * T::TT : T::TT, T::CC,
-             T::NSTAGE, T::QMAX, T::MINB);
+             T::NSTAGE, T::QMAX, T::MINB, T::LAZY ? " lazy" : "");
     Variant v;
     v.name = name;
     v.dtype = T::U8 ? DEDISP_U8 : DEDISP_F32;

@@ -119,22 +119,38 @@ TREE = [
     ("uint8_t", 12, 1, 8, 12, 8, 3, 4, 1),  # 96 x 768
     ("uint8_t", 12, 1, 4, 20, 16, 3, 7, 1), # 48 x 1280, q <= 7 (coarse DM grids)
     ("uint8_t", 4, 1, 4, 12, 8, 3, 4, 4),   # 16 x 768, small problems
+    # ---- LAZY = 1 (10th field): upper window quads loaded only on the paths that read them
+    ("float", 16, 1, 4, 20, 20, 3, 3, 1, 1),
+    ("float", 16, 1, 4, 20, 16, 3, 3, 1, 1),
+    ("float", 12, 1, 4, 28, 16, 3, 3, 1, 1),
+    ("float", 12, 1, 5, 20, 16, 3, 3, 1, 1),
+    ("float", 8, 1, 6, 28, 16, 3, 3, 1, 1),
+    ("float", 8, 1, 8, 20, 8, 4, 3, 1, 1),
+    ("uint8_t", 16, 1, 4, 20, 16, 3, 4, 1, 1),
+    ("uint8_t", 12, 1, 4, 28, 8, 3, 4, 1, 1),
+    ("uint8_t", 12, 1, 5, 20, 16, 3, 4, 1, 1),
+    ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1, 1),
 ]
 
 
+def _combo(t):
+    return ("u32" if t[0] == "uint8_t" else "f32", t[3], t[4], t[7], t[9] if len(t) > 9 else 0)
+
+
 def tree_combos():
-    """(element type, DT, TT, QMAX) lattices gen_tree.py must emit."""
-    return sorted({"%s:%d,%d,%d" % ("u32" if t[0] == "uint8_t" else "f32", t[3], t[4], t[7])
-                   for t in TREE})
+    """(element type, DT, TT, QMAX, LAZY) lattices gen_tree.py must emit."""
+    return sorted({"%s:%d,%d,%d,%d" % _combo(t) for t in TREE})
 
 
 def units():
-    """[(unit name, C++ expression making the Variant)] in registry order: generic, lds, tree."""
+    """[(unit name, C++ expression making the Variant, generated lattice header or None)] in registry
+    order: generic, lds, tree."""
     out = []
     for i, t in enumerate(GENERIC):
-        out.append(("generic%d" % i, "make_generic<%s>()" % t))
+        out.append(("generic%d" % i, "make_generic<%s>()" % t, None))
     for i, t in enumerate(LDS):
-        out.append(("lds%d" % i, "make_tiled<Tile<%s>>()" % ", ".join(str(x) for x in t)))
+        out.append(("lds%d" % i, "make_tiled<Tile<%s>>()" % ", ".join(str(x) for x in t), None))
     for i, t in enumerate(TREE):
-        out.append(("tree%d" % i, "make_tree<TreeTile<%s>>()" % ", ".join(str(x) for x in t)))
+        out.append(("tree%d" % i, "make_tree<TreeTile<%s>>()" % ", ".join(str(x) for x in t),
+                    "tree_gen_%s_%d_%d_%d_%d.cuh" % _combo(t)))
     return out
