@@ -75,21 +75,66 @@ __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
     return T::NSTAGE * tree_stage_bytes<T>(lrow) + 2 * T::NSTAGE * sizeof(uint64_t) + 16 + T::WD * 4;
 }
 
+// Special registers read through opaque moves: what is derived from them is recomputed where it is
+// used (once per chunk, or in the epilogue) instead of being kept in registers across the channel loop,
+// where 80-112 accumulators and a 28-52 register window leave nothing to spare.
+__device__ __forceinline__ uint32_t sreg_tid() { uint32_t v; asm volatile("mov.u32 %0, %%tid.x;" : "=r"(v)); return v; }
+__device__ __forceinline__ uint32_t sreg_ctaid_x() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(v)); return v; }
+__device__ __forceinline__ uint32_t sreg_ctaid_y() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.y;" : "=r"(v)); return v; }
+__device__ __forceinline__ uint32_t sreg_ctaid_z() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.z;" : "=r"(v)); return v; }
+extern __shared__ __align__(128) unsigned char dedisp_smem[];
+__device__ __forceinline__ uint32_t smem_base() {   // shared-window address of the dynamic allocation
+    return (uint32_t)__cvta_generic_to_shared(dedisp_smem);   // a constant to ptxas: costs no register
+}
+
+// mbarriers by shared-window address (the ring's barriers sit at the start of the allocation)
+__device__ __forceinline__ void mbar_arrive_s(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_s(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
+// Layout of the dynamic shared memory, as shared-window byte offsets from its start.
+template <typename T> struct TreeSmem {
+    static constexpr uint32_t FULL = 0, EMPTY = T::NSTAGE * 8;
+    static constexpr uint32_t STAGES = (2 * T::NSTAGE * 8 + 15) & ~15u;
+};
+
 // Issue the copies of chunk k into its stage (called by one whole warp; lane l < CC stages channel
-// k*CC + l: its row span and its WD descriptors).  `rows` is the beam's staged-element matrix
-// [C][pitch]: the fp32 input itself, or the uint8 plan's pair workspace.
+// k*CC + l: its row span and its WD descriptors).  The beam's staged-element matrix [C][pitch] is the
+// fp32 input itself, or the uint8 plan's pair workspace.  Everything is recomputed from the kernel
+// arguments and the block indices (see sreg_*): nothing of it lives across the channel loop.
 template <typename T>
-__device__ __forceinline__ void tree_issue(const KArgs &a, const typename T::Stg *rows, int pitch,
-                                           const uint32_t *desc, int descpitch, int k, int lane,
-                                           int T0, int dm_lo, int g_lo, unsigned char *stages,
-                                           size_t sbytes, size_t data_bytes, uint64_t *full) {
-    const int s = k % T::NSTAGE;
+__device__ __forceinline__ void tree_issue(const KArgs &a, const uint32_t *desc, int descpitch, int k) {
+    const int lane = sreg_tid() & 31;
+    const int dm_lo = sreg_ctaid_x() * T::DMS_CTA, g_lo = sreg_ctaid_x() * T::WD;
+    const int T0 = sreg_ctaid_y() * T::HALF;
+    const int pitch = T::U8 ? a.pair_pitch : a.in_pitch;
+    const typename T::Stg *rows =
+        (const typename T::Stg *)(T::U8 ? (const void *)a.pairs : a.in) + (size_t)sreg_ctaid_z() * a.C * pitch;
+    const uint32_t sbytes = (uint32_t)tree_stage_bytes<T>(a.lrow);
+    const uint32_t data_bytes = (uint32_t)T::CC * a.lrow * 4;
+    const uint32_t base = smem_base();
+    const uint32_t st = base + TreeSmem<T>::STAGES + (uint32_t)(k % T::NSTAGE) * sbytes;
+    const uint32_t full = base + TreeSmem<T>::FULL + (uint32_t)(k % T::NSTAGE) * 8;
     const int c = k * T::CC + lane;
     uint32_t bytes = 0;
     // ragged last chunk: the descriptor row after its last channel ends the channel loop
     const int ncc = a.C - k * T::CC;
     if (ncc < T::CC && lane < T::WD)
-        reinterpret_cast<uint32_t *>(stages + (size_t)s * sbytes + data_bytes)[ncc * T::WD + lane] = 0u;
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(st + data_bytes + (uint32_t)(ncc * T::WD + lane) * 4), "r"(0u)
+                     : "memory");
     if (lane < T::CC && c < a.C) {
         const int32_t *trow = a.shiftT + (size_t)c * a.dpitch + dm_lo;
         const int smin = trow[0], smax = trow[T::DMS_CTA - 1];
@@ -99,17 +144,24 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const typename T::Stg
         int len = (end - g0 + T::AL - 1) & ~(T::AL - 1);
         len = len < a.lrow ? len : a.lrow;
         len = len > 0 ? len : 0;
-        unsigned char *st = stages + (size_t)s * sbytes;
         const uint32_t nb = (uint32_t)len * 4;
-        if (nb) bulk_g2s(st + (size_t)lane * a.lrow * 4, rows + (size_t)c * pitch + g0, nb, &full[s]);
-        bulk_g2s(st + data_bytes + (size_t)lane * T::WD * 4, desc + (size_t)c * descpitch + g_lo,
-                 T::WD * 4, &full[s]);
+        if (nb)
+            asm volatile(
+                "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                    "r"(st + (uint32_t)lane * a.lrow * 4), "l"(rows + (size_t)c * pitch + g0), "r"(nb), "r"(full)
+                : "memory");
+        asm volatile(
+            "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+                "r"(st + data_bytes + (uint32_t)lane * T::WD * 4), "l"(desc + (size_t)c * descpitch + g_lo),
+            "r"((uint32_t)T::WD * 4), "r"(full)
+            : "memory");
         bytes = nb + T::WD * 4;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
     __syncwarp();  // the terminator row is written before lane 0's (releasing) arrive
-    if (lane == 0) mbar_arrive_expect_tx(&full[s], bytes);
+    if (lane == 0)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full), "r"(bytes) : "memory");
 }
 
 // grid: x = DM tiles (fastest: CTAs resident together share input time ranges in L2), y = time
@@ -119,66 +171,53 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
                                                              int descpitch) {
     typedef typename T::Elem Elem;
     typedef typename T::Acc Acc;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw);
-    uint64_t *empty = full + T::NSTAGE;
-    unsigned char *stages = smem_raw + ((2 * T::NSTAGE * sizeof(uint64_t) + 15) & ~(size_t)15);
-    const size_t sbytes = tree_stage_bytes<T>(a.lrow);
-    const size_t data_bytes = (size_t)T::CC * a.lrow * 4;
-
-    // Everything derived from the warp index -- the warp's DM group, its descriptors, every lattice
-    // test -- is warp-uniform: the lattice branches never diverge.
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int dm_lo = blockIdx.x * T::DMS_CTA;
-    const int g_lo = blockIdx.x * T::WD;
-    const int T0 = blockIdx.y * T::HALF;
-    const int nchunks = (a.C + T::CC - 1) / T::CC;
-    // staged rows: fp32 input [B][C][in_pitch], or the pair workspace [B][C][pair_pitch]
-    const int pitch = T::U8 ? a.pair_pitch : a.in_pitch;
-    const typename T::Stg *rows_g =
-        (const typename T::Stg *)(T::U8 ? (const void *)a.pairs : a.in) + (size_t)blockIdx.z * a.C * pitch;
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < T::NSTAGE; ++s) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], T::NW);
+    {
+        uint64_t *full = reinterpret_cast<uint64_t *>(dedisp_smem);
+        uint64_t *empty = full + T::NSTAGE;
+        if (threadIdx.x == 0) {
+            for (int s = 0; s < T::NSTAGE; ++s) {
+                mbar_init(&full[s], 1);
+                mbar_init(&empty[s], T::NW);
+            }
+            mbar_fence_init();
         }
-        mbar_fence_init();
+        // the terminator descriptor row of every stage (row CC; never overwritten by the copies)
+        const size_t sbytes = tree_stage_bytes<T>(a.lrow);
+        if (threadIdx.x < T::NSTAGE * T::WD)
+            reinterpret_cast<uint32_t *>(dedisp_smem + TreeSmem<T>::STAGES + (size_t)(threadIdx.x / T::WD) * sbytes +
+                                         (size_t)T::CC * a.lrow * 4)[T::CC * T::WD + threadIdx.x % T::WD] = 0u;
     }
-    // the terminator descriptor row of every stage (row CC; never overwritten by the copies)
-    if (threadIdx.x < T::NSTAGE * T::WD)
-        reinterpret_cast<uint32_t *>(stages + (size_t)(threadIdx.x / T::WD) * sbytes + data_bytes)
-            [T::CC * T::WD + threadIdx.x % T::WD] = 0u;
     __syncthreads();
+    const int nchunks = (a.C + T::CC - 1) / T::CC;
     // prologue: warp 0 fills the first NSTAGE-1 stages
     constexpr int AHEAD = T::NSTAGE - 1;
-    if (warp == 0)
-        for (int k = 0; k < AHEAD && k < nchunks; ++k)
-            tree_issue<T>(a, rows_g, pitch, desc, descpitch, k, lane, T0, dm_lo, g_lo, stages, sbytes,
-                          data_bytes, full);
+    if (threadIdx.x < 32)
+        for (int k = 0; k < AHEAD && k < nchunks; ++k) tree_issue<T>(a, desc, descpitch, k);
 
-    const int g = warp % T::WD;                  // DM group
-    const int tw = (warp / T::WD) * 32 * T::TT;  // first element of the warp's time chunk
     Elem acc[T::DT][T::TT];
 #pragma unroll
     for (int j = 0; j < T::DT; ++j)
 #pragma unroll
         for (int k = 0; k < T::TT; ++k) acc[j][k] = 0;
 
-    Acc *out = (Acc *)a.out + (size_t)blockIdx.z * a.D * a.S;
-    const int dm0 = dm_lo + g * T::DT;
-    const int t0 = T0 + tw + lane * T::TT;       // the thread's first element (sample / pair index)
+    // Everything derived from the warp index -- the warp's DM group, its descriptors, every lattice
+    // test -- is warp-uniform: the lattice branches never diverge.
 
     // uint8 input: add the 16-bit counters into the uint32 output (the first flush stores) and clear
     // them.  Every output element belongs to exactly one thread, so the read-modify-write needs no
     // atomics.  All loads of one (DM, half) are issued before the first add: TT/4 in flight.
     auto flush = [&](bool first) {
         if constexpr (T::U8) {
+            const uint32_t tid = sreg_tid();
+            const int warp = tid >> 5, lane = tid & 31;
+            const int dm0 = sreg_ctaid_x() * T::DMS_CTA + (warp % T::WD) * T::DT;
+            const int t0 = sreg_ctaid_y() * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
+            uint32_t *out = reinterpret_cast<uint32_t *>(a.out) + (size_t)sreg_ctaid_z() * a.D * a.S;
             const bool vec = (a.S & 3) == 0;
 #pragma unroll
             for (int j = 0; j < T::DT; ++j) {
                 if (dm0 + j < a.D) {
-                    uint32_t *o = reinterpret_cast<uint32_t *>(out) + (size_t)(dm0 + j) * a.S;
+                    uint32_t *o = out + (size_t)(dm0 + j) * a.S;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         // low half: outputs t < S2; high half: outputs S2 + t < S
@@ -224,40 +263,46 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     // The warps flush at different chunks (so that the others keep the pipes busy meanwhile): warp w
     // when (k + 1 + phase_w) is a multiple of FLUSH_CHUNKS.  No counter runs longer than FLUSH_CHUNKS
     // chunks (<= 256 channels) between two flushes.
-    const int phase = T::U8 ? (warp * T::FLUSH_CHUNKS) / T::NW : 0;
     bool flushed = false;
 
-    // Loop constants pinned in registers (an opaque move: otherwise they are re-read from the constant
-    // bank and moved into a register in every channel of the loop below).
+    // What the channel loop keeps in registers besides the accumulators: the thread's place in a staged
+    // row, the warp's descriptor column, the row pitch, and for uint8 the two pipe-pinning constants
+    // (opaque moves: otherwise they are re-read from the constant bank in every channel).
     uint32_t lrow_b, zero, one;
     asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
     asm volatile("mov.u32 %0, %1;" : "=r"(zero) : "r"(a.zero));
     asm volatile("mov.u32 %0, %1;" : "=r"(one) : "r"(a.one));
-    const uint32_t stages_s = smem_u32(stages);
-    const uint32_t my_row = (uint32_t)(tw + lane * T::TT) * 4;      // the thread's place in a row
-    const uint32_t my_desc = (uint32_t)data_bytes + (uint32_t)g * 4;  // the warp's descriptor column
 
     for (int k = 0; k < nchunks; ++k) {
-        const int s = k % T::NSTAGE;
-        mbar_wait(&full[s], (k / T::NSTAGE) & 1);
-        const uint32_t st = stages_s + (uint32_t)s * (uint32_t)sbytes;
-        if constexpr (T::U8)
-            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
-                                                                         lrow_b, zero, one);
-        else
-            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, st + my_row, st + my_desc,
-                                                                         lrow_b);
+        const uint32_t s = k % T::NSTAGE;
+        mbar_wait_s(smem_base() + TreeSmem<T>::FULL + s * 8, (k / T::NSTAGE) & 1);
+        {
+            // the thread's place in a staged row and the warp's descriptor column of this stage
+            // (recomputed per chunk: two registers the channel loop does not have to spare)
+            const uint32_t t = sreg_tid();
+            const uint32_t warp = t >> 5, lane = t & 31;
+            const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
+            const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
+            const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
+            if constexpr (T::U8)
+                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b,
+                                                                                      zero, one);
+            else
+                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
+        }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[s]);
+        const uint32_t tid = sreg_tid();
+        if ((tid & 31) == 0) mbar_arrive_s(smem_base() + TreeSmem<T>::EMPTY + s * 8);
         // producer duty, rotating over the warps (step a4): refill the most recently released
         // stage, which the other warps have normally left by now
         const int kk = k + AHEAD;
-        if (kk < nchunks && warp == k % T::NW) {
-            if (kk >= T::NSTAGE) mbar_wait(&empty[kk % T::NSTAGE], ((kk / T::NSTAGE) - 1) & 1);
-            tree_issue<T>(a, rows_g, pitch, desc, descpitch, kk, lane, T0, dm_lo, g_lo, stages,
-                          sbytes, data_bytes, full);
+        if (kk < nchunks && (int)(tid >> 5) == k % T::NW) {
+            if (kk >= T::NSTAGE)
+                mbar_wait_s(smem_base() + TreeSmem<T>::EMPTY + (kk % T::NSTAGE) * 8, ((kk / T::NSTAGE) - 1) & 1);
+            tree_issue<T>(a, desc, descpitch, kk);
         }
         if constexpr (T::U8) {
+            const int phase = ((int)(tid >> 5) * T::FLUSH_CHUNKS) / T::NW;
             if ((k + 1 + phase) % T::FLUSH_CHUNKS == 0 && k + 1 < nchunks) {
                 flush(!flushed);
                 flushed = true;
@@ -270,6 +315,11 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
         flush(!flushed);
     } else {
         // each thread writes TT consecutive samples of each of its DMs
+        const uint32_t tid = sreg_tid();
+        const int warp = tid >> 5, lane = tid & 31;
+        const int dm0 = sreg_ctaid_x() * T::DMS_CTA + (warp % T::WD) * T::DT;
+        const int t0 = sreg_ctaid_y() * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
+        Acc *out = (Acc *)a.out + (size_t)sreg_ctaid_z() * a.D * a.S;
         const bool vec = (a.S & 3) == 0 && t0 + T::TT <= a.S;
 #pragma unroll
         for (int j = 0; j < T::DT; ++j) {
