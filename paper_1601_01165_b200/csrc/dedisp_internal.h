@@ -85,6 +85,7 @@ struct Variant {
     int cc;           // channel-chunk depth (channels per pipeline stage)
     int stages;
     int qmax;         // KIND_TREE: largest slope class q_c the variant's lattice covers
+    int lazy = 0;     // KIND_TREE: upper window quads loaded on demand (gen_tree.py)
     int threads;
     // Fills lrow/smem, returns whether the variant supports the plan.
     VariantFit (*fit)(const Variant &, const PlanShape &, int span_cta);

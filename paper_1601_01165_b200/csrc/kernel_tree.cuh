@@ -270,8 +270,8 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     // (opaque moves: otherwise they are re-read from the constant bank in every channel).
     uint32_t lrow_b, zero, one;
     asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
-    asm volatile("mov.u32 %0, %1;" : "=r"(zero) : "r"(a.zero));
-    asm volatile("mov.u32 %0, %1;" : "=r"(one) : "r"(a.one));
+    zero = a.zero;
+    one = a.one;
 
     for (int k = 0; k < nchunks; ++k) {
         const uint32_t s = k % T::NSTAGE;

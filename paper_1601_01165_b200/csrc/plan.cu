@@ -143,7 +143,7 @@ static int prepare_variant(dedisp_plan *pl, int v) {
 // Adds per clock and SM the tree tiles sustain on B200 (round-2 measurements on apertif / survey8, tile
 // and wave quantisation divided out): {uint8?, DT, samples per thread and DM, warps per CTA, rate}.
 // Tiles not listed fall back to a formula.  Only the untuned default uses this; dedisp_tune measures.
-static double tree_rate(bool u8, int dt, int tt, int warps, int cc) {
+static double tree_rate(bool u8, int dt, int tt, int warps, int cc, int lazy) {
     static const struct { int u8, dt, tt, warps; double rate; } kRates[] = {
         {0, 4, 28, 12, 76}, {0, 5, 20, 12, 74}, {0, 6, 28, 8, 71}, {0, 6, 12, 16, 68}, {0, 4, 20, 12, 66},
         {0, 4, 44, 8, 65},  {0, 5, 12, 16, 63}, {0, 5, 36, 8, 63}, {0, 8, 20, 8, 62},  {0, 6, 12, 12, 60},
@@ -159,6 +159,7 @@ static double tree_rate(bool u8, int dt, int tt, int warps, int cc) {
         const double tile = (double)dt * tt;
         rate = (tile >= 100 ? (warps >= 12 ? 62 : 58) : tile >= 72 ? 52 : 42) * (u8 ? 1.4 : 1.0);
     }
+    if (lazy) rate *= u8 ? 1.045 : 1.035;  // upper window quads on demand: ~10 % fewer shared-memory wavefronts
     return rate * (cc >= 12 ? 1.0 : 0.93);  // 8-channel stages: more chunk bookkeeping per add
 }
 
@@ -178,7 +179,7 @@ static int heuristic_variant(const dedisp_plan *pl) {
         const double tile = (double)x.dt * x.tt;
         double rate, need, occ;
         if (x.kind == KIND_TREE) {
-            rate = tree_rate(pl->dtype == DEDISP_U8, x.dt, x.tt, x.threads / 32, x.cc);
+            rate = tree_rate(pl->dtype == DEDISP_U8, x.dt, x.tt, x.threads / 32, x.cc, x.lazy);
             need = 8;
             occ = x.threads <= 128 ? 4 : (x.threads <= 256 && tile <= 48) ? 2 : 1;
         } else if (x.kind == KIND_LDS) {

@@ -160,6 +160,7 @@ Variant make_tree() {
     v.cc = T::CC;
     v.stages = T::NSTAGE;
     v.qmax = T::QMAX;
+    v.lazy = T::LAZY;
     v.threads = T::THREADS;
     v.fit = tree_fit<T>;
     v.launch = tree_launch<T>;

@@ -120,16 +120,28 @@ TREE = [
     ("uint8_t", 12, 1, 4, 20, 16, 3, 7, 1), # 48 x 1280, q <= 7 (coarse DM grids)
     ("uint8_t", 4, 1, 4, 12, 8, 3, 4, 4),   # 16 x 768, small problems
     # ---- LAZY = 1 (10th field): upper window quads loaded only on the paths that read them
-    ("float", 16, 1, 4, 20, 20, 3, 3, 1, 1),
+    ("float", 16, 1, 4, 20, 20, 3, 3, 1, 1),   # 64 x 640
     ("float", 16, 1, 4, 20, 16, 3, 3, 1, 1),
-    ("float", 12, 1, 4, 28, 16, 3, 3, 1, 1),
-    ("float", 12, 1, 5, 20, 16, 3, 3, 1, 1),
-    ("float", 8, 1, 6, 28, 16, 3, 3, 1, 1),
-    ("float", 8, 1, 8, 20, 8, 4, 3, 1, 1),
-    ("uint8_t", 16, 1, 4, 20, 16, 3, 4, 1, 1),
-    ("uint8_t", 12, 1, 4, 28, 8, 3, 4, 1, 1),
-    ("uint8_t", 12, 1, 5, 20, 16, 3, 4, 1, 1),
-    ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1, 1),
+    ("float", 16, 1, 4, 20, 12, 4, 3, 1, 1),
+    ("float", 12, 1, 4, 28, 16, 3, 3, 1, 1),   # 48 x 896
+    ("float", 12, 1, 4, 28, 12, 4, 3, 1, 1),
+    ("float", 12, 1, 5, 20, 16, 3, 3, 1, 1),   # 60 x 640
+    ("float", 12, 1, 4, 20, 16, 3, 4, 1, 1),   # 48 x 640, q <= 4
+    ("float", 16, 1, 6, 12, 16, 3, 4, 1, 1),   # 96 x 384
+    ("float", 16, 1, 4, 12, 16, 3, 4, 1, 1),   # 64 x 384
+    ("float", 8, 1, 6, 28, 16, 3, 3, 1, 1),    # 48 x 896, 8 warps
+    ("float", 8, 1, 8, 20, 8, 4, 3, 1, 1),     # 64 x 640, 8 warps
+    ("float", 12, 1, 4, 20, 16, 3, 7, 1, 1),   # 48 x 640, q <= 7 (coarse DM grids)
+    ("float", 8, 1, 4, 12, 8, 3, 4, 2, 1),     # 32 x 384, 2 CTAs/SM (small problems)
+    ("uint8_t", 16, 1, 4, 20, 16, 3, 4, 1, 1),  # 64 x 1280
+    ("uint8_t", 16, 1, 4, 20, 12, 4, 4, 1, 1),
+    ("uint8_t", 16, 1, 4, 20, 12, 3, 4, 1, 1),
+    ("uint8_t", 12, 1, 4, 20, 16, 3, 4, 1, 1),  # 48 x 1280
+    ("uint8_t", 12, 1, 4, 28, 8, 3, 4, 1, 1),   # 48 x 1792
+    ("uint8_t", 12, 1, 5, 20, 16, 3, 4, 1, 1),  # 60 x 1280
+    ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1, 1),  # 80 x 768
+    ("uint8_t", 16, 1, 4, 12, 16, 3, 4, 1, 1),  # 64 x 768
+    ("uint8_t", 12, 1, 4, 20, 16, 3, 7, 1, 1),  # 48 x 1280, q <= 7
 ]
 
 
