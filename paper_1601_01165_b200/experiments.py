@@ -46,7 +46,8 @@ def gflops(setup, ms):
 
 
 def short(name):
-    return name.split(" DMsxsamples")[0] + "," + name.split("CTA,")[1].split(" outputs")[0]
+    return (name.split(" DMsxsamples")[0] + "," + name.split("CTA,")[1].split(" outputs")[0]
+            + (" lazy" if name.endswith(" lazy") else ""))
 
 
 def sweep():
