@@ -35,7 +35,6 @@ struct KArgs {
     int S2;                  // pair y holds samples y and y + S2 (about S/2, multiple of 4)
     const uint32_t *desc;    // KIND_TREE: [C][descpitch] descriptors for the variant's tile
     int descpitch;
-    uint32_t zero, one;      // 0 and 1 the compiler cannot see (uint8 tree kernels, gen_tree.py)
 };
 
 // Per-variant numbers derived from the plan's shift table at plan creation.

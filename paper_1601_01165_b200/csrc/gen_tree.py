@@ -57,9 +57,7 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
     o = []
     wnmax = wn(dt, tt, qmax)
     ct, pt, rc = CTYPE[typ]
-    # u32: two warp-uniform run-time constants (0 and 1) that pin the pipe of each add, see tree_add
-    xdecl = ", uint32_t zero, uint32_t one" if typ == "u32" else ""
-    xargs = ", zero, one" if typ == "u32" else ""
+    xdecl = xargs = ""   # (an earlier uint8 lattice passed two pipe-pinning constants through here)
     o.append("template <> struct TreeStep<%s, %d, %d, %d, %d> {" % (ct, dt, tt, qmax, lazy))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
     # One function per slope class q: the channel loop over a run of channels of that class.  The loop
@@ -187,21 +185,19 @@ __device__ __forceinline__ void tree_add(float (&acc)[TT], const float (&w)[WN])
 }
 // uint8 input: acc and w hold two 16-bit counters / samples per word, so one 32-bit add does two adds
 // whatever the offset.  Integer adds issue at half rate on either of two pipes: IADD3 on the integer
-// pipe, IMAD on the FMA pipe.  Left to itself ptxas turns three of four adds into IMAD.IADD (84
-// lanes/clk/SM measured); alternating a three-input IADD3 (+ a run-time zero) with an IMAD (x a
-// run-time one), neither of which it can rewrite, reaches 115 (profiles/r02_microbench.md).
+// pipe, IMAD on the FMA pipe.  Left to itself ptxas turns three of four plain adds into IMAD.IADD (84
+// lanes/clk/SM measured).  Writing two neighbouring adds as ONE carry chain (add.cc / addc) pins one to
+// each pipe, IADD3 + IMAD.X, at 116 lanes/clk/SM (profiles/r02_microbench.md, run 5), without the two
+// run-time constants an earlier version needed to keep ptxas from rewriting the adds.  The carry is
+// always zero: a word's upper counter stays below 2^16 between flushes, so the low add cannot overflow
+// (only lanes past the staged data can, and what they and their right neighbours compute is never stored).
 template <int R, int TT, int WN>
-__device__ __forceinline__ void tree_add(uint32_t (&acc)[TT], const uint32_t (&w)[WN], uint32_t zero,
-                                         uint32_t one) {
-    static_assert(R + TT <= WN, "window too short");
+__device__ __forceinline__ void tree_add(uint32_t (&acc)[TT], const uint32_t (&w)[WN]) {
+    static_assert(R + TT <= WN && TT % 2 == 0, "window too short");
 #pragma unroll
-    for (int k = 0; k < TT; ++k) {
-        if (k % 2 == 0)
-            asm volatile("{.reg .u32 t; add.u32 t, %1, %2; add.u32 %0, %0, t;}"
-                         : "+r"(acc[k]) : "r"(w[R + k]), "r"(zero));
-        else
-            asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc[k]) : "r"(w[R + k]), "r"(one));
-    }
+    for (int k = 0; k < TT; k += 2)
+        asm volatile("add.cc.u32 %0, %0, %2; addc.u32 %1, %1, %3;"
+                     : "+r"(acc[k]), "+r"(acc[k + 1]) : "r"(w[R + k]), "r"(w[R + k + 1]));
 }
 """
 

@@ -265,13 +265,10 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     // chunks (<= 256 channels) between two flushes.
     bool flushed = false;
 
-    // What the channel loop keeps in registers besides the accumulators: the thread's place in a staged
-    // row, the warp's descriptor column, the row pitch, and for uint8 the two pipe-pinning constants
-    // (opaque moves: otherwise they are re-read from the constant bank in every channel).
-    uint32_t lrow_b, zero, one;
+    // What the channel loop keeps in registers besides the accumulators: the row pitch (an opaque move:
+    // otherwise it is re-read from the constant bank in every channel).
+    uint32_t lrow_b;
     asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
-    zero = a.zero;
-    one = a.one;
 
     for (int k = 0; k < nchunks; ++k) {
         const uint32_t s = k % T::NSTAGE;
@@ -284,11 +281,7 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
             const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
             const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
-            if constexpr (T::U8)
-                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b,
-                                                                                      zero, one);
-            else
-                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
+            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
         }
         __syncwarp();
         const uint32_t tid = sreg_tid();

@@ -358,7 +358,6 @@ static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void
     a.C = plan->C; a.D = plan->D; a.S = (int)plan->S; a.in_pitch = plan->in_pitch;
     a.dpitch = plan->dpitch; a.lrow = f.lrow;
     a.pairs = plan->d_pairs; a.pair_pitch = plan->pair_pitch; a.S2 = plan->S2;
-    a.zero = 0; a.one = 1;
     const TreeTable *tt = x.kind == KIND_TREE ? plan->tree.find(x.dt, x.dms_cta) : nullptr;
     if (x.kind == KIND_TREE && !tt) return DEDISP_ERR_INVALID_ARG;  // variant was never prepared
     a.desc = tt ? tt->d_desc : nullptr;

@@ -142,6 +142,7 @@ TREE = [
     ("uint8_t", 16, 1, 5, 12, 16, 3, 4, 1, 1),  # 80 x 768
     ("uint8_t", 16, 1, 4, 12, 16, 3, 4, 1, 1),  # 64 x 768
     ("uint8_t", 12, 1, 4, 20, 16, 3, 7, 1, 1),  # 48 x 1280, q <= 7
+    ("uint8_t", 16, 1, 4, 20, 16, 3, 3, 1, 1),  # 64 x 1280, q <= 3
 ]
 
 

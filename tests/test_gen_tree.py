@@ -119,10 +119,11 @@ def test_chunk_loop_dispatches_one_hot_slope_classes():
     assert "uint32_t d = tree_desc<0>(ds);" in chunk
     for q in range(4):
         assert "if (d & %du) { loop_q%d<WD>(acc, rows, ds, d, lrow_b); goto NEXT; }" % (0x10000 << q, q) in chunk
-    # the uint8 lattices carry the two run-time constants that pin the pipe of each add
+    # the uint8 lattices have the same shape (their adds are carry chains: gen_tree.py HEADER)
     text8 = gen_tree.emit(4, 28, 4, "u32")
-    assert "loop_q4<WD>(acc, rows, ds, d, lrow_b, zero, one)" in text8.split("void chunk(")[1]
-    assert "tree_add<7, 28>(acc[1], w, zero, one);" in text8
+    assert "loop_q4<WD>(acc, rows, ds, d, lrow_b)" in text8.split("void chunk(")[1]
+    assert "tree_add<7, 28>(acc[1], w);" in text8
+    assert "add.cc.u32 %0, %0, %2; addc.u32 %1, %1, %3;" in gen_tree.HEADER
 
 
 def test_descriptor_layout_constants():
