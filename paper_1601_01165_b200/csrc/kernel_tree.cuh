@@ -270,36 +270,46 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     uint32_t lrow_b;
     asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
 
-    for (int k = 0; k < nchunks; ++k) {
-        const uint32_t s = k % T::NSTAGE;
-        mbar_wait_s(smem_base() + TreeSmem<T>::FULL + s * 8, (k / T::NSTAGE) & 1);
-        {
-            // the thread's place in a staged row and the warp's descriptor column of this stage
-            // (recomputed per chunk: two registers the channel loop does not have to spare)
-            const uint32_t t = sreg_tid();
-            const uint32_t warp = t >> 5, lane = t & 31;
-            const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
-            const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
-            const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
-            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
-        }
-        __syncwarp();
-        const uint32_t tid = sreg_tid();
-        if ((tid & 31) == 0) mbar_arrive_s(smem_base() + TreeSmem<T>::EMPTY + s * 8);
-        // producer duty, rotating over the warps (step a4): refill the most recently released
-        // stage, which the other warps have normally left by now
-        const int kk = k + AHEAD;
-        if (kk < nchunks && (int)(tid >> 5) == k % T::NW) {
-            if (kk >= T::NSTAGE)
-                mbar_wait_s(smem_base() + TreeSmem<T>::EMPTY + (kk % T::NSTAGE) * 8, ((kk / T::NSTAGE) - 1) & 1);
-            tree_issue<T>(a, desc, descpitch, kk);
+    // The chunk loop runs in segments that end where this warp flushes its counters (uint8) or at the last
+    // chunk: the flush sits OUTSIDE the inner loop, so that its register needs (20 registers of old sums per
+    // DM half) do not make ptxas shuffle two dozen accumulators at every chunk's entry and exit.
+    int k = 0;
+    int kend = nchunks;
+    if constexpr (T::U8) kend = T::FLUSH_CHUNKS - ((int)(sreg_tid() >> 5) * T::FLUSH_CHUNKS) / T::NW;
+    while (k < nchunks) {
+        if (kend > nchunks) kend = nchunks;
+#pragma unroll 1
+        for (; k < kend; ++k) {
+            const uint32_t s = k % T::NSTAGE;
+            mbar_wait_s(smem_base() + TreeSmem<T>::FULL + s * 8, (k / T::NSTAGE) & 1);
+            {
+                // the thread's place in a staged row and the warp's descriptor column of this stage
+                // (recomputed per chunk: two registers the channel loop does not have to spare)
+                const uint32_t t = sreg_tid();
+                const uint32_t warp = t >> 5, lane = t & 31;
+                const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
+                const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
+                const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
+                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
+            }
+            __syncwarp();
+            const uint32_t tid = sreg_tid();
+            if ((tid & 31) == 0) mbar_arrive_s(smem_base() + TreeSmem<T>::EMPTY + s * 8);
+            // producer duty, rotating over the warps (step a4): refill the most recently released
+            // stage, which the other warps have normally left by now
+            const int kk = k + AHEAD;
+            if (kk < nchunks && (int)(tid >> 5) == k % T::NW) {
+                if (kk >= T::NSTAGE)
+                    mbar_wait_s(smem_base() + TreeSmem<T>::EMPTY + (kk % T::NSTAGE) * 8, ((kk / T::NSTAGE) - 1) & 1);
+                tree_issue<T>(a, desc, descpitch, kk);
+            }
         }
         if constexpr (T::U8) {
-            const int phase = ((int)(tid >> 5) * T::FLUSH_CHUNKS) / T::NW;
-            if ((k + 1 + phase) % T::FLUSH_CHUNKS == 0 && k + 1 < nchunks) {
+            if (k < nchunks) {
                 flush(!flushed);
                 flushed = true;
             }
+            kend += T::FLUSH_CHUNKS;
         }
     }
 
