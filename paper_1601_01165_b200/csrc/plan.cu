@@ -145,10 +145,10 @@ static int prepare_variant(dedisp_plan *pl, int v) {
 // Tiles not listed fall back to a formula.  Only the untuned default uses this; dedisp_tune measures.
 static double tree_rate(bool u8, int dt, int tt, int warps, int cc, int lazy) {
     static const struct { int u8, dt, tt, warps; double rate; } kRates[] = {
-        {0, 4, 28, 12, 76}, {0, 5, 20, 12, 74}, {0, 6, 28, 8, 71}, {0, 6, 12, 16, 68}, {0, 4, 20, 12, 66},
+        {0, 4, 28, 12, 76}, {0, 4, 20, 16, 75}, {0, 5, 20, 12, 74}, {0, 6, 28, 8, 71}, {0, 6, 12, 16, 68}, {0, 4, 20, 12, 66},
         {0, 4, 44, 8, 65},  {0, 5, 12, 16, 63}, {0, 5, 36, 8, 63}, {0, 8, 20, 8, 62},  {0, 6, 12, 12, 60},
         {0, 4, 28, 8, 60},  {0, 4, 12, 16, 60}, {0, 6, 20, 8, 57}, {0, 8, 12, 12, 57}, {0, 4, 36, 8, 62},
-        {1, 5, 24, 16, 108}, {1, 4, 40, 12, 107}, {1, 5, 40, 12, 100}, {1, 4, 24, 16, 101}, {1, 6, 24, 12, 87},
+        {1, 4, 40, 16, 110}, {1, 5, 24, 16, 108}, {1, 4, 40, 12, 107}, {1, 5, 40, 12, 100}, {1, 4, 24, 16, 101}, {1, 6, 24, 12, 87},
         {1, 6, 24, 16, 84},  {1, 4, 56, 12, 92},  {1, 8, 24, 12, 79},  {1, 4, 72, 8, 82},   {1, 6, 56, 8, 64},
         {1, 8, 40, 8, 47},
     };
@@ -159,7 +159,7 @@ static double tree_rate(bool u8, int dt, int tt, int warps, int cc, int lazy) {
         const double tile = (double)dt * tt;
         rate = (tile >= 100 ? (warps >= 12 ? 62 : 58) : tile >= 72 ? 52 : 42) * (u8 ? 1.4 : 1.0);
     }
-    if (lazy) rate *= u8 ? 1.045 : 1.035;  // upper window quads on demand: ~10 % fewer shared-memory wavefronts
+    if (lazy) rate *= u8 ? 1.06 : 1.035;  // upper window quads on demand: ~10 % fewer shared-memory wavefronts
     return rate * (cc >= 12 ? 1.0 : 0.93);  // 8-channel stages: more chunk bookkeeping per add
 }
 
