@@ -1,6 +1,7 @@
 """Shipped tuning results (step a8): winners of dedisp_tune on a B200, one text line per
 (GPU, setup), in the format dedisp_tune appends.  `python -m paper_1601_01165_b200.tuning`
-re-tunes the five BASELINE.json configs on the current GPU and rewrites the file."""
+re-tunes the five BASELINE.json configs (or the ones named on the command line, keeping the other
+entries) on the current GPU and rewrites the file."""
 from __future__ import annotations
 
 import os
@@ -36,6 +37,14 @@ def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 8) -> None:
         for v, t in sorted(ms.items(), key=lambda kv: kv[1]):
             print("%-10s %9.4f ms  %s" % (name, t, dedisp.variant_name(v)))
         plan.destroy()
+    # keep the shipped entries of setups that were not retuned (a partial retune must not drop them)
+    fresh = [l for l in open(tmp).read().splitlines() if l.strip()]
+    keys = {l.split("\t")[0] for l in fresh}
+    kept = []
+    if os.path.exists(out_path):
+        kept = [l for l in open(out_path).read().splitlines() if l.strip() and l.split("\t")[0] not in keys]
+    with open(tmp, "w") as f:
+        f.write("\n".join(kept + fresh) + "\n")
     os.replace(tmp, out_path)
 
 
