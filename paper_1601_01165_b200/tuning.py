@@ -17,6 +17,15 @@ def apply_shipped(plan, nr_beams: int = 1) -> bool:
     return os.path.exists(SHIPPED) and plan.load_tuning(SHIPPED, nr_beams)
 
 
+def merge_entries(old_text: str, new_text: str) -> str:
+    """The cache file after a (partial) retune: the old entries whose key (text before the first tab) was
+    not retuned, then the new ones."""
+    fresh = [l for l in new_text.splitlines() if l.strip()]
+    keys = {l.split("\t")[0] for l in fresh}
+    kept = [l for l in old_text.splitlines() if l.strip() and l.split("\t")[0] not in keys]
+    return "\n".join(kept + fresh) + "\n"
+
+
 def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 8) -> None:
     import torch
 
@@ -37,14 +46,11 @@ def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 8) -> None:
         for v, t in sorted(ms.items(), key=lambda kv: kv[1]):
             print("%-10s %9.4f ms  %s" % (name, t, dedisp.variant_name(v)))
         plan.destroy()
-    # keep the shipped entries of setups that were not retuned (a partial retune must not drop them)
-    fresh = [l for l in open(tmp).read().splitlines() if l.strip()]
-    keys = {l.split("\t")[0] for l in fresh}
-    kept = []
-    if os.path.exists(out_path):
-        kept = [l for l in open(out_path).read().splitlines() if l.strip() and l.split("\t")[0] not in keys]
+    old = open(out_path).read() if os.path.exists(out_path) else ""
+    with open(tmp) as f:
+        merged = merge_entries(old, f.read())
     with open(tmp, "w") as f:
-        f.write("\n".join(kept + fresh) + "\n")
+        f.write(merged)
     os.replace(tmp, out_path)
 
 

@@ -46,3 +46,14 @@ def test_traffic_table_names_shipped_winners_and_existing_summaries():
         assert int(r["compulsory_bytes"]) == bench.compulsory_bytes(
             wl.CONFIGS[name], {"apertif": 26707, "lofar": 272797, "survey8": 68987, "batch40": 26707}[name])
     assert bench.ncu_traffic("tiny", "x") == (None, None)
+
+
+def test_partial_retune_keeps_the_other_entries():
+    from paper_1601_01165_b200 import tuning
+    old = "k1\tvariant a\t1 ms\nk2\tvariant b\t2 ms\n"
+    new = "k2\tvariant c\t1.5 ms\nk3\tvariant d\t3 ms\n"
+    assert tuning.merge_entries(old, new) == "k1\tvariant a\t1 ms\nk2\tvariant c\t1.5 ms\nk3\tvariant d\t3 ms\n"
+    assert tuning.merge_entries("", new) == new
+    shipped = open(tuning.SHIPPED).read()
+    assert tuning.merge_entries(shipped, "") == shipped       # five entries, unique keys
+    assert len({l.split("\t")[0] for l in shipped.splitlines()}) == 5

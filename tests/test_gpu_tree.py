@@ -133,3 +133,24 @@ def test_long_shift_setup_uses_a_staged_kernel(dd):
         ran += 1
     assert ran >= 3
     plan.destroy()
+
+
+@pytest.mark.parametrize("base", ["apertif", "survey8"])
+def test_lazy_window_twins_are_bit_identical(dd, base):
+    """A LAZY lattice loads the same words later, it does not change a single add or its order: on Gaussian
+    fp32 data (where the tolerance against the oracle would hide a changed order) every lazy variant must
+    reproduce its up-front twin bit for bit; likewise on uint8."""
+    import torch
+    s = wl.scaled(wl.CONFIGS[base], name=base + "_twins", nr_dms=333, nr_samples=3001)
+    plan, table, x, d_in = make_case(dd, s)
+    names = {dd.variant_name(v): v for v in tree_variants(dd, plan)}
+    pairs = [(v, names[n[:-len(" lazy")]]) for n, v in names.items()
+             if n.endswith(" lazy") and n[:-len(" lazy")] in names]
+    assert len(pairs) >= 4
+    for lazy, plain in pairs:
+        a = out_buffer(s, fill=-1 if s.in_dtype == wl.U8 else float("nan"))
+        b = out_buffer(s, fill=-2 if s.in_dtype == wl.U8 else float("nan"))
+        plan.execute_variant(lazy, d_in, a, nr_beams=s.nr_beams)
+        plan.execute_variant(plain, d_in, b, nr_beams=s.nr_beams)
+        assert torch.equal(a.view(torch.int32), b.view(torch.int32)), dd.variant_name(lazy)
+    plan.destroy()
