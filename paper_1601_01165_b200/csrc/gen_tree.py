@@ -57,7 +57,6 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
     o = []
     wnmax = wn(dt, tt, qmax)
     ct, pt, rc = CTYPE[typ]
-    xdecl = xargs = ""   # (an earlier uint8 lattice passed two pipe-pinning constants through here)
     o.append("template <> struct TreeStep<%s, %d, %d, %d, %d> {" % (ct, dt, tt, qmax, lazy))
     o.append("    static constexpr int WNMAX = %d;" % wnmax)
     # One function per slope class q: the channel loop over a run of channels of that class.  The loop
@@ -94,7 +93,7 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
         o.append("    // channel; d: that descriptor (warp-uniform).  Returns at the first channel of another class.")
         o.append("    template <int WD>")
         o.append("    static __device__ __forceinline__ void loop_q%d(%s (&acc)[%d][%d], uint32_t &rows, "
-                 "uint32_t &ds, uint32_t &d, uint32_t lrow_b%s) {" % (q, ct, dt, tt, xdecl))
+                 "uint32_t &ds, uint32_t &d, uint32_t lrow_b) {" % (q, ct, dt, tt))
         o.append("        %s w[%d];" % (ct, n))
         o.append("        uint32_t dn, p;")
         for line in enter:
@@ -108,7 +107,7 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
                     edge = range(max(have, need(r + q, tt)) + 1, need(r + q + 1, tt) + 1)  # by bit = 1 only
                     for m in both:
                         o.append("        " + loads[m])
-                    o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
+                    o.append("        tree_add<%d, %d>(acc[%d], w);" % (r, tt, j))
                     if len(edge):
                         o.append("        if (d & %du) { %s goto N_%d_%d; } else goto N_%d_%d;"
                                  % (1 << (BIT_SHIFT + j), " ".join(loads[m] for m in edge), j + 1, r + q + 1,
@@ -117,7 +116,7 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
                         o.append("        if (d & %du) goto N_%d_%d; else goto N_%d_%d;"
                                  % (1 << (BIT_SHIFT + j), j + 1, r + q + 1, j + 1, r + q))
                 else:
-                    o.append("        tree_add<%d, %d>(acc[%d], w%s);" % (r, tt, j, xargs))
+                    o.append("        tree_add<%d, %d>(acc[%d], w);" % (r, tt, j))
                     # the loop step, one copy per last node (the comment keeps the copies from being
                     # merged back into one shared block behind a jump)
                     o.append('        asm volatile("// step q%d r%d");' % (q, r))
@@ -137,12 +136,12 @@ def emit(dt: int, tt: int, qmax: int, typ: str = "f32", lazy: int = 0) -> str:
     o.append("    // a zero row after the last channel); lrow_b: bytes per staged row.")
     o.append("    template <int WD>")
     o.append("    static __device__ __forceinline__ void chunk(%s (&acc)[%d][%d], uint32_t rows, "
-             "uint32_t ds, uint32_t lrow_b%s) {" % (ct, dt, tt, xdecl))
+             "uint32_t ds, uint32_t lrow_b) {" % (ct, dt, tt))
     o.append("        uint32_t d = tree_desc<0>(ds);")
     o.append("    NEXT:")
     for q in range(qmax + 1):
-        o.append("        if (d & %du) { loop_q%d<WD>(acc, rows, ds, d, lrow_b%s); goto NEXT; }"
-                 % (1 << (Q_SHIFT + q), q, xargs))
+        o.append("        if (d & %du) { loop_q%d<WD>(acc, rows, ds, d, lrow_b); goto NEXT; }"
+                 % (1 << (Q_SHIFT + q), q))
     o.append("    }")
     o.append("};")
     return "\n".join(o)
