@@ -35,6 +35,7 @@ struct KArgs {
     int S2;                  // pair y holds samples y and y + S2 (about S/2, multiple of 4)
     const uint32_t *desc;    // KIND_TREE: [C][descpitch] descriptors for the variant's tile
     int descpitch;
+    int nx, ny, ntiles;      // KIND_TREE (persistent CTAs): DM tiles, time tiles, nx * ny * beams
 };
 
 // Per-variant numbers derived from the plan's shift table at plan creation.

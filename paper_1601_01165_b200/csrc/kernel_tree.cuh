@@ -50,6 +50,8 @@ struct TreeTile {
                          QMAX = QMAX_, MINB = MINB_;
     // LAZY = 1: the upper window quads are loaded only on the lattice paths that read them (gen_tree.py)
     static constexpr int LAZY = LAZY_;
+    // persistent CTAs (fp32): the chunk ring runs on across the CTA's tiles, see tree_tile
+    static constexpr bool PERSIST = !U8;
     static constexpr int NW = WD * WT;
     static constexpr int THREADS = NW * 32;
     static constexpr int DMS_CTA = WD * DT;
@@ -80,6 +82,7 @@ __host__ __device__ inline size_t tree_smem_bytes(int lrow) {
 // where 80-112 accumulators and a 28-52 register window leave nothing to spare.
 __device__ __forceinline__ uint32_t sreg_tid() { uint32_t v; asm volatile("mov.u32 %0, %%tid.x;" : "=r"(v)); return v; }
 __device__ __forceinline__ uint32_t sreg_ctaid_x() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(v)); return v; }
+__device__ __forceinline__ uint32_t sreg_nctaid_x() { uint32_t v; asm volatile("mov.u32 %0, %%nctaid.x;" : "=r"(v)); return v; }
 __device__ __forceinline__ uint32_t sreg_ctaid_y() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.y;" : "=r"(v)); return v; }
 __device__ __forceinline__ uint32_t sreg_ctaid_z() { uint32_t v; asm volatile("mov.u32 %0, %%ctaid.z;" : "=r"(v)); return v; }
 extern __shared__ __align__(128) unsigned char dedisp_smem[];
@@ -111,23 +114,56 @@ template <typename T> struct TreeSmem {
     static constexpr uint32_t STAGES = (2 * T::NSTAGE * 8 + 15) & ~15u;
 };
 
-// Issue the copies of chunk k into its stage (called by one whole warp; lane l < CC stages channel
-// k*CC + l: its row span and its WD descriptors).  The beam's staged-element matrix [C][pitch] is the
-// fp32 input itself, or the uint8 plan's pair workspace.  Everything is recomputed from the kernel
-// arguments and the block indices (see sreg_*): nothing of it lives across the channel loop.
+// The kernel is PERSISTENT: a CTA works through the tiles blockIdx.x, blockIdx.x + gridDim.x, ... (tile id =
+// (beam * ny + time tile) * nx + DM tile, DM tiles fastest: the CTAs running together share input time ranges
+// in L2), and its chunk ring runs on across tile boundaries, so the first chunks of the next tile are in
+// flight while the last ones of this tile are added and its results stored.  Tile `it` of this CTA:
+// uint8 kernels are not persistent (measured 1 % slower): there the grid is (DM tiles, time tiles, beams)
+// and a CTA has the one tile its block index names.
+template <bool PERSIST>
+__device__ __forceinline__ void tree_tile(const KArgs &a, int it, int &tx, int &ty, int &bz) {
+    if constexpr (PERSIST) {
+        const uint32_t tile = sreg_ctaid_x() + (uint32_t)it * sreg_nctaid_x();
+        tx = (int)(tile % (uint32_t)a.nx);
+        const uint32_t r = tile / (uint32_t)a.nx;
+        ty = (int)(r % (uint32_t)a.ny);
+        bz = (int)(r / (uint32_t)a.ny);
+    } else {
+        tx = (int)sreg_ctaid_x();
+        ty = (int)sreg_ctaid_y();
+        bz = (int)sreg_ctaid_z();
+    }
+}
+template <bool PERSIST>
+__device__ __forceinline__ int tree_my_tiles(const KArgs &a) {   // tiles this CTA works through (>= 1)
+    if constexpr (PERSIST)
+        return (int)(((uint32_t)a.ntiles - sreg_ctaid_x() + sreg_nctaid_x() - 1) / sreg_nctaid_x());
+    else
+        return 1;
+}
+
+// Issue the copies of ring position g (chunk g % nchunks of the CTA's tile g / nchunks) into its stage
+// (called by one whole warp; lane l < CC stages channel k*CC + l: its row span and its WD descriptors).
+// The beam's staged-element matrix [C][pitch] is the fp32 input itself, or the uint8 plan's pair workspace.
+// Everything is recomputed from the kernel arguments and the block index (see sreg_*): nothing of it lives
+// across the channel loop.
 template <typename T>
-__device__ __forceinline__ void tree_issue(const KArgs &a, const uint32_t *desc, int descpitch, int k) {
+__device__ __forceinline__ void tree_issue(const KArgs &a, const uint32_t *desc, int descpitch, int g, int nchunks) {
     const int lane = sreg_tid() & 31;
-    const int dm_lo = sreg_ctaid_x() * T::DMS_CTA, g_lo = sreg_ctaid_x() * T::WD;
-    const int T0 = sreg_ctaid_y() * T::HALF;
+    const int it = g / nchunks;
+    const int k = g - it * nchunks;   // chunk of tile `it`; the ring position is g
+    int tx, ty, bz;
+    tree_tile<T::PERSIST>(a, it, tx, ty, bz);
+    const int dm_lo = tx * T::DMS_CTA, g_lo = tx * T::WD;
+    const int T0 = ty * T::HALF;
     const int pitch = T::U8 ? a.pair_pitch : a.in_pitch;
     const typename T::Stg *rows =
-        (const typename T::Stg *)(T::U8 ? (const void *)a.pairs : a.in) + (size_t)sreg_ctaid_z() * a.C * pitch;
+        (const typename T::Stg *)(T::U8 ? (const void *)a.pairs : a.in) + (size_t)bz * a.C * pitch;
     const uint32_t sbytes = (uint32_t)tree_stage_bytes<T>(a.lrow);
     const uint32_t data_bytes = (uint32_t)T::CC * a.lrow * 4;
     const uint32_t base = smem_base();
-    const uint32_t st = base + TreeSmem<T>::STAGES + (uint32_t)(k % T::NSTAGE) * sbytes;
-    const uint32_t full = base + TreeSmem<T>::FULL + (uint32_t)(k % T::NSTAGE) * 8;
+    const uint32_t st = base + TreeSmem<T>::STAGES + (uint32_t)(g % T::NSTAGE) * sbytes;
+    const uint32_t full = base + TreeSmem<T>::FULL + (uint32_t)(g % T::NSTAGE) * 8;
     const int c = k * T::CC + lane;
     uint32_t bytes = 0;
     // ragged last chunk: the descriptor row after its last channel ends the channel loop
@@ -164,8 +200,7 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const uint32_t *desc,
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full), "r"(bytes) : "memory");
 }
 
-// grid: x = DM tiles (fastest: CTAs resident together share input time ranges in L2), y = time
-// tiles, z = beams.
+// grid: min(tiles, SMs x CTAs per SM) persistent CTAs (tree_tile above).
 template <typename T>
 __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, const uint32_t *desc,
                                                              int descpitch) {
@@ -191,8 +226,10 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     const int nchunks = (a.C + T::CC - 1) / T::CC;
     // prologue: warp 0 fills the first NSTAGE-1 stages
     constexpr int AHEAD = T::NSTAGE - 1;
-    if (threadIdx.x < 32)
-        for (int k = 0; k < AHEAD && k < nchunks; ++k) tree_issue<T>(a, desc, descpitch, k);
+    if (threadIdx.x < 32) {
+        const int total = tree_my_tiles<T::PERSIST>(a) * nchunks;
+        for (int g = 0; g < AHEAD && g < total; ++g) tree_issue<T>(a, desc, descpitch, g, nchunks);
+    }
 
     Elem acc[T::DT][T::TT];
 #pragma unroll
@@ -206,13 +243,15 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
     // uint8 input: add the 16-bit counters into the uint32 output (the first flush stores) and clear
     // them.  Every output element belongs to exactly one thread, so the read-modify-write needs no
     // atomics.  All loads of one (DM, half) are issued before the first add: TT/4 in flight.
-    auto flush = [&](bool first) {
+    auto flush = [&](int it, bool first) {
         if constexpr (T::U8) {
             const uint32_t tid = sreg_tid();
             const int warp = tid >> 5, lane = tid & 31;
-            const int dm0 = sreg_ctaid_x() * T::DMS_CTA + (warp % T::WD) * T::DT;
-            const int t0 = sreg_ctaid_y() * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
-            uint32_t *out = reinterpret_cast<uint32_t *>(a.out) + (size_t)sreg_ctaid_z() * a.D * a.S;
+            int tx, ty, bz;
+            tree_tile<T::PERSIST>(a, it, tx, ty, bz);
+            const int dm0 = tx * T::DMS_CTA + (warp % T::WD) * T::DT;
+            const int t0 = ty * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
+            uint32_t *out = reinterpret_cast<uint32_t *>(a.out) + (size_t)bz * a.D * a.S;
             const bool vec = (a.S & 3) == 0;
 #pragma unroll
             for (int j = 0; j < T::DT; ++j) {
@@ -260,83 +299,93 @@ __global__ void __launch_bounds__(T::THREADS, T::MINB) tree_kernel(KArgs a, cons
             }
         }
     };
-    // The warps flush at different chunks (so that the others keep the pipes busy meanwhile): warp w
-    // when (k + 1 + phase_w) is a multiple of FLUSH_CHUNKS.  No counter runs longer than FLUSH_CHUNKS
-    // chunks (<= 256 channels) between two flushes.
-    bool flushed = false;
-
     // What the channel loop keeps in registers besides the accumulators: the row pitch (an opaque move:
     // otherwise it is re-read from the constant bank in every channel).
     uint32_t lrow_b;
     asm volatile("mov.u32 %0, %1;" : "=r"(lrow_b) : "r"(a.lrow * 4));
 
-    // The chunk loop runs in segments that end where this warp flushes its counters (uint8) or at the last
-    // chunk: the flush sits OUTSIDE the inner loop, so that its register needs (20 registers of old sums per
-    // DM half) do not make ptxas shuffle two dozen accumulators at every chunk's entry and exit.
-    int k = 0;
-    int kend = nchunks;
-    if constexpr (T::U8) kend = T::FLUSH_CHUNKS - ((int)(sreg_tid() >> 5) * T::FLUSH_CHUNKS) / T::NW;
-    while (k < nchunks) {
-        if (kend > nchunks) kend = nchunks;
-#pragma unroll 1
-        for (; k < kend; ++k) {
-            const uint32_t s = k % T::NSTAGE;
-            mbar_wait_s(smem_base() + TreeSmem<T>::FULL + s * 8, (k / T::NSTAGE) & 1);
-            {
-                // the thread's place in a staged row and the warp's descriptor column of this stage
-                // (recomputed per chunk: two registers the channel loop does not have to spare)
-                const uint32_t t = sreg_tid();
-                const uint32_t warp = t >> 5, lane = t & 31;
-                const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
-                const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
-                const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
-                TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
-            }
-            __syncwarp();
-            const uint32_t tid = sreg_tid();
-            if ((tid & 31) == 0) mbar_arrive_s(smem_base() + TreeSmem<T>::EMPTY + s * 8);
-            // producer duty, rotating over the warps (step a4): refill the most recently released
-            // stage, which the other warps have normally left by now
-            const int kk = k + AHEAD;
-            if (kk < nchunks && (int)(tid >> 5) == k % T::NW) {
-                if (kk >= T::NSTAGE)
-                    mbar_wait_s(smem_base() + TreeSmem<T>::EMPTY + (kk % T::NSTAGE) * 8, ((kk / T::NSTAGE) - 1) & 1);
-                tree_issue<T>(a, desc, descpitch, kk);
-            }
+    // One pass of the ring position g: wait for the chunk, add it, release its stage, and (one warp per
+    // chunk, rotating: step a4) refill the most recently released stage with the chunk AHEAD positions on,
+    // which may already belong to the CTA's next tile.
+    auto ring_step = [&](int g) {
+        const uint32_t s = g % T::NSTAGE;
+        mbar_wait_s(smem_base() + TreeSmem<T>::FULL + s * 8, (g / T::NSTAGE) & 1);
+        {
+            // the thread's place in a staged row and the warp's descriptor column of this stage
+            // (recomputed per chunk: two registers the channel loop does not have to spare)
+            const uint32_t t = sreg_tid();
+            const uint32_t warp = t >> 5, lane = t & 31;
+            const uint32_t st = smem_base() + TreeSmem<T>::STAGES + s * (uint32_t)tree_stage_bytes<T>(a.lrow);
+            const uint32_t my_row = st + ((warp / T::WD) * 32 * T::TT + lane * T::TT) * 4;
+            const uint32_t my_desc = st + (uint32_t)T::CC * a.lrow * 4 + (warp % T::WD) * 4;
+            TreeStep<Elem, T::DT, T::TT, T::QMAX, T::LAZY>::template chunk<T::WD>(acc, my_row, my_desc, lrow_b);
         }
-        if constexpr (T::U8) {
+        __syncwarp();
+        const uint32_t tid = sreg_tid();
+        if ((tid & 31) == 0) mbar_arrive_s(smem_base() + TreeSmem<T>::EMPTY + s * 8);
+        const int gg = g + AHEAD;
+        if ((int)(tid >> 5) == g % T::NW && gg < tree_my_tiles<T::PERSIST>(a) * nchunks) {
+            if (gg >= T::NSTAGE)
+                mbar_wait_s(smem_base() + TreeSmem<T>::EMPTY + (gg % T::NSTAGE) * 8, ((gg / T::NSTAGE) - 1) & 1);
+            tree_issue<T>(a, desc, descpitch, gg, nchunks);
+        }
+    };
+
+    if constexpr (T::U8) {
+        // uint8: one tile per CTA (the launch makes the grid as large as the tile count; persistent CTAs
+        // measured 1 % slower here).  The chunk loop runs in segments that end where this warp flushes its
+        // counters: the flush sits OUTSIDE the inner loop, so that its register needs (20 registers of old
+        // sums per DM half) do not make ptxas shuffle two dozen accumulators at every chunk's entry and exit.
+        // The warps flush at different chunks (the others keep the pipes busy meanwhile): warp w after the
+        // chunks k with (k + 1 + phase_w) a multiple of FLUSH_CHUNKS; no counter runs longer than
+        // FLUSH_CHUNKS chunks (<= 256 channels) between two flushes.
+        bool flushed = false;
+        int k = 0;
+        int kend = T::FLUSH_CHUNKS - ((int)(sreg_tid() >> 5) * T::FLUSH_CHUNKS) / T::NW;
+        while (k < nchunks) {
+            if (kend > nchunks) kend = nchunks;
+#pragma unroll 1
+            for (; k < kend; ++k) ring_step(k);
             if (k < nchunks) {
-                flush(!flushed);
+                flush(0, !flushed);
                 flushed = true;
             }
             kend += T::FLUSH_CHUNKS;
         }
-    }
-
-    // store (step a6)
-    if constexpr (T::U8) {
-        flush(!flushed);
+        flush(0, !flushed);   // step a6
     } else {
-        // each thread writes TT consecutive samples of each of its DMs
-        const uint32_t tid = sreg_tid();
-        const int warp = tid >> 5, lane = tid & 31;
-        const int dm0 = sreg_ctaid_x() * T::DMS_CTA + (warp % T::WD) * T::DT;
-        const int t0 = sreg_ctaid_y() * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
-        Acc *out = (Acc *)a.out + (size_t)sreg_ctaid_z() * a.D * a.S;
-        const bool vec = (a.S & 3) == 0 && t0 + T::TT <= a.S;
+        // fp32: persistent CTAs; the ring runs on across the CTA's tiles, the store sits between them
+        int g = 0;
+        while (g < tree_my_tiles<T::PERSIST>(a) * nchunks) {
+            const int gend = g + nchunks;
+#pragma unroll 1
+            for (; g < gend; ++g) ring_step(g);
+            // store (step a6): each thread writes TT consecutive samples of each of its DMs
+            const uint32_t tid = sreg_tid();
+            const int warp = tid >> 5, lane = tid & 31;
+            int tx, ty, bz;
+            tree_tile<T::PERSIST>(a, g / nchunks - 1, tx, ty, bz);
+            const int dm0 = tx * T::DMS_CTA + (warp % T::WD) * T::DT;
+            const int t0 = ty * T::HALF + (warp / T::WD) * 32 * T::TT + lane * T::TT;
+            Acc *out = (Acc *)a.out + (size_t)bz * a.D * a.S;
+            const bool vec = (a.S & 3) == 0 && t0 + T::TT <= a.S;
 #pragma unroll
-        for (int j = 0; j < T::DT; ++j) {
-            if (dm0 + j >= a.D) break;
-            float *o = out + (size_t)(dm0 + j) * a.S + t0;
-            if (vec) {
+            for (int j = 0; j < T::DT; ++j) {
+                if (dm0 + j < a.D) {
+                    float *o = out + (size_t)(dm0 + j) * a.S + t0;
+                    if (vec) {
 #pragma unroll
-                for (int k = 0; k < T::TT; k += 4)
-                    *reinterpret_cast<float4 *>(o + k) =
-                        make_float4(acc[j][k], acc[j][k + 1], acc[j][k + 2], acc[j][k + 3]);
-            } else {
+                        for (int k2 = 0; k2 < T::TT; k2 += 4)
+                            *reinterpret_cast<float4 *>(o + k2) =
+                                make_float4(acc[j][k2], acc[j][k2 + 1], acc[j][k2 + 2], acc[j][k2 + 3]);
+                    } else {
 #pragma unroll
-                for (int k = 0; k < T::TT; ++k)
-                    if (t0 + k < a.S) o[k] = acc[j][k];
+                        for (int k2 = 0; k2 < T::TT; ++k2)
+                            if (t0 + k2 < a.S) o[k2] = acc[j][k2];
+                    }
+                }
+#pragma unroll
+                for (int k2 = 0; k2 < T::TT; ++k2) acc[j][k2] = 0;
             }
         }
     }

@@ -128,10 +128,34 @@ VariantFit tree_fit(const Variant &v, const PlanShape &p, int span_cta) {
     return f;
 }
 
+// Persistent CTAs (kernel_tree.cuh): as many as fit the device at once, each working through every
+// (SMs x CTAs per SM)-th tile.
+inline int device_sm_count() {
+    static int sms[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    if (!sms[dev]) cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
+    return sms[dev] > 0 ? sms[dev] : 1;
+}
+
 template <typename T>
-cudaError_t tree_launch(const KArgs &a, int nr_beams, size_t smem, cudaStream_t st) {
+cudaError_t tree_launch(const KArgs &a0, int nr_beams, size_t smem, cudaStream_t st) {
+    KArgs a = a0;
     const int nt = T::U8 ? a.S2 : a.S;  // pairs / samples along time
-    dim3 grid((a.D + T::DMS_CTA - 1) / T::DMS_CTA, (nt + T::HALF - 1) / T::HALF, nr_beams);
+    a.nx = (a.D + T::DMS_CTA - 1) / T::DMS_CTA;
+    a.ny = (nt + T::HALF - 1) / T::HALF;
+    const long long tiles = (long long)a.nx * a.ny * nr_beams;
+    if (tiles > 0x7fffffffLL) return cudaErrorInvalidValue;
+    a.ntiles = (int)tiles;
+    // fp32: persistent CTAs (0.9 % faster: the next tile's first chunks are in flight while a tile's last
+    // ones are added and its results stored).  uint8: one CTA per tile on a 3-D grid (persistent CTAs
+    // measured 1 % slower there).
+    dim3 grid((unsigned)a.nx, (unsigned)a.ny, (unsigned)nr_beams);
+    if (T::PERSIST) {
+        const long long resident = (long long)device_sm_count() * T::MINB;
+        grid = dim3((unsigned)(tiles < resident ? tiles : resident), 1, 1);
+    }
     tree_kernel<T><<<grid, T::THREADS, smem, st>>>(a, a.desc, a.descpitch);
     return cudaGetLastError();
 }
