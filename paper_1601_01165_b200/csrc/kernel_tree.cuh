@@ -168,9 +168,13 @@ __device__ __forceinline__ void tree_issue(const KArgs &a, const uint32_t *desc,
     uint32_t bytes = 0;
     // ragged last chunk: the descriptor row after its last channel ends the channel loop
     const int ncc = a.C - k * T::CC;
-    if (ncc < T::CC && lane < T::WD)
+    // (a generic-proxy store into a stage the bulk copies of a later chunk overwrite again: the proxy fence
+    // orders it before them)
+    if (ncc < T::CC && lane < T::WD) {
         asm volatile("st.shared.u32 [%0], %1;" ::"r"(st + data_bytes + (uint32_t)(ncc * T::WD + lane) * 4), "r"(0u)
                      : "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
     if (lane < T::CC && c < a.C) {
         const int32_t *trow = a.shiftT + (size_t)c * a.dpitch + dm_lo;
         const int smin = trow[0], smax = trow[T::DMS_CTA - 1];
