@@ -154,3 +154,15 @@ def test_lazy_window_twins_are_bit_identical(dd, base):
         plan.execute_variant(plain, d_in, b, nr_beams=s.nr_beams)
         assert torch.equal(a.view(torch.int32), b.view(torch.int32)), dd.variant_name(lazy)
     plan.destroy()
+
+
+def test_persistent_ctas_cross_tiles_and_beams_on_every_fp32_variant(dd):
+    """The fp32 tree kernels run as persistent CTAs whose chunk ring runs on across tiles.  The scaled
+    configs of the other tests have fewer tiles than the GPU has SMs; here every compiled fp32 tree tile
+    gets more than 2 x 148 tiles over two beams (so every CTA crosses tile and beam boundaries), with a
+    channel count that leaves a ragged last chunk for every stage depth (70 = 3 x 20 + 10 = 4 x 16 + 6 =
+    5 x 12 + 10 = 8 x 8 + 6), ragged DM and time tiles, integer-valued data: exact."""
+    s = wl.scaled(wl.APERTIF, name="persist", nr_channels=70, channel_bw_MHz=300.0 / 70, nr_dms=700,
+                  nr_samples=9001, nr_beams=2, values="int16")
+    n, q = run_tree(dd, s, exact=True)
+    assert n >= 30 and q >= 3
