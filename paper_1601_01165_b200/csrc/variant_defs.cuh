@@ -75,10 +75,13 @@ cudaError_t tiled_launch(const KArgs &a, int nr_beams, size_t smem, cudaStream_t
     return cudaGetLastError();
 }
 
+// The attribute belongs to the kernel, not to a plan: it is set to the most any plan may ask for (the
+// fit functions refuse more than kMaxSmem), so that preparing the variant for a second, smaller plan does
+// not lower the limit under a live plan that needs more.
 template <typename T>
-cudaError_t tiled_prepare(size_t smem) {
+cudaError_t tiled_prepare(size_t) {
     return cudaFuncSetAttribute(tiled_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)smem);
+                                (int)kMaxSmem);
 }
 
 // name: "lds_<dtype>: DMSxSAMPLES DMsxsamples/CTA, dtxtt outputs/thread, ccN sN bN" (static storage).
@@ -161,9 +164,9 @@ cudaError_t tree_launch(const KArgs &a0, int nr_beams, size_t smem, cudaStream_t
 }
 
 template <typename T>
-cudaError_t tree_prepare(size_t smem) {
+cudaError_t tree_prepare(size_t) {   // see tiled_prepare
     return cudaFuncSetAttribute(tree_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)smem);
+                                (int)kMaxSmem);
 }
 
 template <typename T>

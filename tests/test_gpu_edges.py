@@ -80,6 +80,29 @@ def test_execute_is_repeatable_and_stream_ordered(dd):
     plan.destroy()
 
 
+@pytest.mark.parametrize("kind", ["tree_f32", "lds_f32"])
+def test_two_live_plans_of_different_size_on_one_variant(dd, kind):
+    """The large-shared-memory attribute belongs to the kernel, not to a plan: selecting the variant for a
+    second plan with shorter staged rows must not lower it under the first plan (whose launch then failed
+    with 'invalid argument')."""
+    big = wl.scaled(wl.APERTIF, name="two_big", nr_channels=96, channel_bw_MHz=300.0 / 96, nr_dms=700,
+                    nr_samples=3000, values="int16")
+    small = wl.scaled(big, name="two_small", nr_dms=64, dm_step=0.02)
+    pa, ta, xa, da = make_case(dd, big)
+    va = [v for v in pa.supported_variants() if dd.variant_name(v).startswith(kind)]
+    pb, tb, xb, db = make_case(dd, small)
+    common = [v for v in va if pb.variant_supported(v)]
+    assert common
+    pa.set_variant(common[-1])
+    pb.set_variant(common[-1])     # smaller shift span: fewer bytes of dynamic shared memory
+    for s, plan, x, table, d_in in ((big, pa, xa, ta, da), (small, pb, xb, tb, db), (big, pa, xa, ta, da)):
+        d_out = out_buffer(s, fill=float("nan"))
+        plan.execute(d_in, d_out)
+        assert np.array_equal(to_host(s, d_out).astype(np.float64), oracle.dedisperse(x, table, s.nr_samples))
+    pa.destroy()
+    pb.destroy()
+
+
 @pytest.mark.parametrize("u8", [False, True])
 def test_first_execute_of_a_fresh_plan_can_be_captured_into_a_cuda_graph(dd, u8):
     """dedisp_execute promises no allocation, no host sync and no function-attribute call (all done
