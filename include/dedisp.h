@@ -134,6 +134,49 @@ int dedisp_execute_variant(const dedisp_plan *plan, int variant, const void *d_i
                            int nr_beams, void *stream);
 
 /*
+ * dedisp_execute_static_scratch -- dedisp_execute for callers that cannot allocate device memory.
+ *
+ * The uint8 register-window kernels (tree_u8 variants) read the input through a scratch copy in which
+ * every row is repacked as pairs of samples (see dedisp_plan_reserve).  dedisp_execute keeps that copy
+ * in a plan-owned buffer from cudaMalloc.  Not every caller can have such a buffer: a process whose
+ * free device memory already belongs to a pool allocator (PyTorch's caching allocator, RMM) gets
+ * "out of memory" from cudaMalloc although the pool has room; a real-time block loop cannot afford
+ * cudaMalloc / cudaFree, which serialise the device and stall every other stream; and while another
+ * thread captures a CUDA graph in the global capture mode, an allocation call is refused and breaks that
+ * capture.  For them this entry point keeps the scratch in a fixed array inside the library image
+ * (dedisp_static_scratch_bytes() bytes, 16 MiB; every GPU that loads the library holds that much from
+ * load to process exit, used or not).  The call launches kernels and does nothing else: no cudaMalloc,
+ * cudaFree, memset, copy, synchronisation or function-attribute call.  The plan itself still comes from
+ * dedisp_plan_create, which does allocate (tables, and the workspace this call leaves untouched):
+ * create plans in set-up code, before the phase in which allocation is off limits.
+ *
+ *   plan, d_in, d_out, nr_beams, stream: exactly as for dedisp_execute; same results, bit for bit.
+ *   The plan must be a U8 plan whose selected variant (DEDISP_VARIANT) is a tree_u8 kernel; other
+ *   plans use no scratch memory and are refused with INVALID_ARG: call dedisp_execute for them.
+ *   One beam needs nr_channels * PAIR_PITCH * 4 bytes of scratch (PAIR_PITCH = nr_samples / 2 rounded
+ *   up to a multiple of 4, plus MAX_SHIFT, rounded up to 4).  If that exceeds
+ *   dedisp_static_scratch_bytes() the call returns INVALID_ARG and dedisp_last_error() names both
+ *   sizes.  A batch goes through the array as many beams at a time as fit, in stream order.
+ *
+ * First call on a device: the library looks up where the array lives on that device
+ * (cudaGetSymbolAddress, once per device, with that device current) and remembers it.  Make this first
+ * call outside any stream capture; later calls skip the lookup.
+ * Sharing: there is ONE array per GPU, shared by every plan, stream and thread of the process, and it
+ * keeps what the last call wrote.  No call depends on those contents (each call rewrites every scratch
+ * word it later reads, padding included, so nothing needs clearing), but two calls whose kernels can
+ * overlap on the GPU (different streams without an event between them) race on the array and
+ * produce garbage.  Order all calls of this entry point on one device with respect to each other.
+ * It does not touch the plan's own workspace, so it may overlap a dedisp_execute on the same plan.
+ * Errors: INVALID_ARG (as dedisp_execute; not a tree_u8 plan; scratch need beyond the maximum;
+ * device ordinal >= 64), CUDA (symbol lookup or launch error).
+ */
+int dedisp_execute_static_scratch(const dedisp_plan *plan, const void *d_in, void *d_out, int nr_beams,
+                                  void *stream);
+
+/* Size in bytes of the static scratch array dedisp_execute_static_scratch works in (per GPU). */
+int64_t dedisp_static_scratch_bytes(void);
+
+/*
  * dedisp_execute_host -- the same computation for HOST buffers (end-to-end path; the paper keeps
  * data resident on the device, so this is a convenience, not the hot path):
  *   h_in : HOST, [nr_beams][nr_channels][IN_PITCH], borrowed (pinned memory copies fastest);

@@ -111,6 +111,7 @@ cudaError_t pack_pairs(const uint8_t *d_in, uint32_t *d_pairs, int nr_beams, int
                        int pair_pitch, int S2, cudaStream_t st);
 
 void set_last_error(const char *what, cudaError_t e);
+void set_last_error_text(const char *msg);  // a message that is not a CUDA error (dedisp_last_error)
 
 // Three-stage host pipeline of dedisp_execute_host_async (host_pipe.cu).
 struct HostPipe {

@@ -19,6 +19,8 @@ void set_last_error(const char *what, cudaError_t e) {
     snprintf(g_last_error, sizeof g_last_error, "%s: %s", what, cudaGetErrorString(e));
 }
 
+void set_last_error_text(const char *msg) { snprintf(g_last_error, sizeof g_last_error, "%s", msg); }
+
 #include "build/registry_gen.inc"  // generated from variants.py: kVariantMakers[]
 
 const std::vector<Variant> &variants() {

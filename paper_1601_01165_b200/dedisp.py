@@ -23,7 +23,7 @@ F32, U8 = 0, 1
 # every symbol include/dedisp.h declares
 SYMBOLS = [
     "dedisp_plan_create", "dedisp_plan_reserve", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
-    "dedisp_execute_variant", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
+    "dedisp_execute_variant", "dedisp_execute_static_scratch", "dedisp_static_scratch_bytes", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
     "dedisp_stream_block_async",
     "dedisp_plan_destroy", "dedisp_variant_count",
     "dedisp_variant_name", "dedisp_variant_supported", "dedisp_plan_set_variant", "dedisp_tune",
@@ -56,6 +56,9 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_execute.argtypes = [vp, vp, vp, ci, vp]
     lib.dedisp_execute_variant.argtypes = [vp, ci, vp, vp, ci, vp]
     lib.dedisp_execute_host.argtypes = [vp, vp, vp, ci, vp]
+    lib.dedisp_execute_static_scratch.argtypes = [vp, vp, vp, ci, vp]
+    lib.dedisp_static_scratch_bytes.argtypes = []
+    lib.dedisp_static_scratch_bytes.restype = i64
     lib.dedisp_execute_host_async.argtypes = [vp, vp, vp, ci]
     lib.dedisp_host_sync.argtypes = [vp]
     lib.dedisp_stream_block_async.argtypes = [vp, vp, i64, vp, i64, i64]
@@ -72,7 +75,7 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_last_error.argtypes = []
     lib.dedisp_last_error.restype = ctypes.c_char_p
     for name in SYMBOLS:
-        if getattr(lib, name).restype is not ctypes.c_char_p:
+        if getattr(lib, name).restype not in (ctypes.c_char_p, i64):
             getattr(lib, name).restype = ci
     _lib = lib
     return lib
@@ -100,6 +103,11 @@ def _stream(stream) -> Optional[int]:
     if stream is None:
         return None
     return int(getattr(stream, "cuda_stream", stream)) or None
+
+
+def static_scratch_bytes() -> int:
+    """dedisp_static_scratch_bytes: size of the fixed scratch array execute_static_scratch works in."""
+    return int(load_library().dedisp_static_scratch_bytes())
 
 
 def variant_count() -> int:
@@ -176,6 +184,16 @@ class Plan:
         _check(self._lib.dedisp_execute_variant(self._h, int(variant), _addr(d_in), _addr(d_out),
                                                 int(nr_beams), _stream(stream)),
                "dedisp_execute_variant")
+
+    def execute_static_scratch(self, d_in, d_out, nr_beams: int = 1, stream=None):
+        """dedisp_execute_static_scratch: execute() for callers that cannot allocate device memory (a
+        pool allocator owns it all, a real-time loop, a thread beside a global-mode graph capture).
+        uint8 plans on a tree_u8 variant only; the pair scratch is a fixed array in the library image
+        instead of the plan's cudaMalloc'ed workspace, so the scratch need is capped
+        (static_scratch_bytes()) and all such calls on one GPU must be ordered with respect to each
+        other.  Same results as execute(), bit for bit.  See include/dedisp.h."""
+        _check(self._lib.dedisp_execute_static_scratch(self._h, _addr(d_in), _addr(d_out), int(nr_beams),
+                                                       _stream(stream)), "dedisp_execute_static_scratch")
 
     def execute_host(self, h_in, h_out, nr_beams: int = 1, stream=None):
         _check(self._lib.dedisp_execute_host(self._h, _addr(h_in), _addr(h_out), int(nr_beams),
