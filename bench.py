@@ -68,6 +68,18 @@ def ncu_traffic(config_name, variant_name):
     return int(d["dram_bytes_per_step"]), d["source"]
 
 
+def resident_bytes_per_beam(s, in_pitch, pair_pitch, vname):
+    """Device bytes one beam keeps resident while it is dedispersed: its input rows, its output, and for
+    the tree_u8 kernels the beam's share of the plan-owned pair workspace (4 bytes per pair,
+    nr_channels x PAIR_PITCH pairs: 273 MB for survey8, 2.6x the input itself).  The 180 GB of a B200
+    divided by this is the memory cap on beams held at once."""
+    esz = 1 if s.in_dtype == wl.U8 else 4
+    n = s.nr_channels * in_pitch * esz + s.nr_dms * s.nr_samples * 4
+    if vname.startswith("tree_u8"):
+        n += s.nr_channels * pair_pitch * 4
+    return n
+
+
 def compulsory_bytes(s, in_samples):
     """Input read once + output written once (north_star)."""
     esz = 1 if s.in_dtype == wl.U8 else 4
@@ -261,7 +273,7 @@ class Case:
         self.s = s
         self.plan = plan = dedisp.Plan(*s.plan_args())
         B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
-        self.in_samples, self.pitch = plan.in_samples, plan.in_pitch
+        self.in_samples, self.pitch, self.pair_pitch = plan.in_samples, plan.in_pitch, plan.pair_pitch
         self.in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32
         self.out_dt = torch.int32 if s.in_dtype == wl.U8 else torch.float32
         esz = 1 if s.in_dtype == wl.U8 else 4
@@ -339,7 +351,7 @@ def report(case, world, total_ms, per, steps, hbm_gbs, sm_max_mhz, peak_kind):
         "ms_per_step": ms_step, "ms_per_step_median": float(np.median(per)), "ms_per_step_min": float(per[0]),
         "value": aggregate_value(adds, world, ms_step * 1e-3), "unit": UNIT, "dtype": dtype_name(s),
         "real_time_factor": rt, "beams_in_real_time": int(np.floor(rt)),
-        "beams_memory_cap": int(180e9 // (case.set_bytes / B)),
+        "beams_memory_cap": int(180e9 // resident_bytes_per_beam(s, case.pitch, case.pair_pitch, case.vname)),
         "roofline": {"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": src, "note": note},
         "hbm_roofline": {"compulsory_bytes": comp, "achieved_gbs": comp / (kern_ms * 1e-3) / 1e9,

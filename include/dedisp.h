@@ -56,7 +56,10 @@ enum {
     DEDISP_NR_SAMPLES = 7,
     DEDISP_IN_DTYPE = 8,
     DEDISP_MAX_STEP = 9,   /* max over (c, i) of shift(c, i+1) - shift(c, i) */
-    DEDISP_RESERVED_BEAMS = 10 /* U8 plans: beams the pair workspace holds (dedisp_plan_reserve); else 0 */
+    DEDISP_RESERVED_BEAMS = 10, /* U8 plans: beams the pair workspace holds (dedisp_plan_reserve); else 0 */
+    DEDISP_PAIR_PITCH = 11 /* U8 plans: 4-byte pairs per row of the pair workspace (nr_samples / 2 rounded up
+                              to 4, plus MAX_SHIFT, rounded up to 4): one beam of workspace or static scratch
+                              takes nr_channels * PAIR_PITCH * 4 bytes; else 0 */
 };
 
 /*

@@ -345,6 +345,7 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value) {
         case DEDISP_IN_DTYPE: *value = plan->dtype; break;
         case DEDISP_MAX_STEP: *value = plan->max_step; break;
         case DEDISP_RESERVED_BEAMS: *value = plan->dtype == DEDISP_U8 ? plan->pairs_beams : 0; break;
+        case DEDISP_PAIR_PITCH: *value = plan->dtype == DEDISP_U8 ? plan->pair_pitch : 0; break;
         default: return DEDISP_ERR_INVALID_ARG;
     }
     return DEDISP_OK;

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
 
 F32, U8 = 0, 1
 (MAX_SHIFT, IN_SAMPLES, IN_PITCH, OUT_PITCH, VARIANT, NR_CHANNELS, NR_DMS, NR_SAMPLES, IN_DTYPE,
- MAX_STEP, RESERVED_BEAMS) = range(11)
+ MAX_STEP, RESERVED_BEAMS, PAIR_PITCH) = range(12)
 
 # every symbol include/dedisp.h declares
 SYMBOLS = [
@@ -164,6 +164,7 @@ class Plan:
     in_dtype = property(lambda self: self.get(IN_DTYPE))
     max_step = property(lambda self: self.get(MAX_STEP))
     reserved_beams = property(lambda self: self.get(RESERVED_BEAMS))
+    pair_pitch = property(lambda self: self.get(PAIR_PITCH))
 
     def reserve(self, nr_beams: int):
         """dedisp_plan_reserve: size the uint8 pair workspace for batches of nr_beams beams."""

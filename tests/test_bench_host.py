@@ -33,6 +33,18 @@ def test_compulsory_bytes_match_the_survey_table():
     assert bench.compulsory_bytes(wl.BATCH40, 26707) == 40 * 273231872
 
 
+def test_memory_cap_counts_the_pair_workspace_of_the_uint8_tree_kernels():
+    # survey8: 106 MB of input + 805 MB of output per beam, and 1536 x (24576 + 19835 -> 44412) x 4 B = 273 MB of
+    # pairs for the tree_u8 kernels only: 152 beams in 180 GB, not the 197 that input + output alone would give
+    in_pitch, pair_pitch = 68992, 44412
+    io = 1536 * in_pitch + 4096 * 49152 * 4
+    tree = bench.resident_bytes_per_beam(wl.SURVEY8, in_pitch, pair_pitch, "tree_u8: 64x1280 ...")
+    assert tree == io + 1536 * pair_pitch * 4 and int(180e9 // tree) == 152
+    assert bench.resident_bytes_per_beam(wl.SURVEY8, in_pitch, pair_pitch, "lds_u8: 16x1024 ...") == io
+    assert int(180e9 // io) == 197
+    assert bench.resident_bytes_per_beam(wl.APERTIF, 26708, 0, "tree_f32: 64x640 ...") == 1024 * 26708 * 4 + 2048 * 20000 * 4
+
+
 def test_traffic_table_names_shipped_winners_and_existing_summaries():
     rows = {r["config"]: r for r in csv.DictReader(open(bench.TRAFFIC_CSV))}
     assert set(rows) == {"apertif", "lofar", "survey8", "batch40"}

@@ -29,6 +29,7 @@ def scratch_need_bytes(plan):
     """include/dedisp.h: one beam needs nr_channels * PAIR_PITCH * 4 bytes."""
     s2 = ((plan.nr_samples + 1) // 2 + 3) & ~3
     pair_pitch = (s2 + plan.max_shift + 3) & ~3
+    assert pair_pitch == plan.pair_pitch
     return plan.nr_channels * pair_pitch * 4
 
 
