@@ -72,8 +72,9 @@ enum {
  * Chooses the kernel variant (tuning cache named by $DEDISP_TUNE_CACHE if set, else a
  * heuristic) and prepares it (function attributes, its descriptor table).  nr_samples = S,
  * output samples per beam.  The plan belongs to the CUDA device that is current at creation;
- * every later call on it must be made with the same device current.  U8 plans also allocate
- * the pair workspace for one beam (dedisp_plan_reserve).
+ * every later call on it must be made with the same device current.  A U8 plan whose selected
+ * variant is a tree_u8 kernel also allocates the pair workspace for one beam (dedisp_plan_reserve);
+ * if there is no memory for it, the plan is created on the best kernel that needs no workspace.
  * Errors: INVALID_ARG (plan == NULL, C/D/S < 1, f_low/bw/rate <= 0 or non-finite,
  * dm_first/dm_step < 0 or non-finite, unknown dtype, or no compiled kernel variant can run the
  * plan); OVERFLOW (shift or S+M > INT32_MAX, or C*255 >= 2^32 for U8); ALLOC; CUDA.  On error
@@ -95,10 +96,16 @@ int dedisp_shift_table(const dedisp_plan *plan, int32_t *host_out);
  * dedisp_plan_reserve -- U8 plans only (a no-op returning OK for F32 plans): the uint8 register-window
  * kernels read the input through a plan-owned device workspace holding every input row as pairs of
  * samples about S/2 apart (two 16-bit counters per 32-bit add; 4 bytes per pair, C * (S/2 + M) pairs
- * per beam).  dedisp_plan_create allocates it for one beam; this call grows it to nr_beams beams so
- * that dedisp_execute runs a whole batch in one kernel launch.  Without it a larger batch still
- * works: dedisp_execute then goes through the workspace as many beams at a time as it holds.
- * Synchronises the device and allocates; never shrinks.  Errors: INVALID_ARG, ALLOC, CUDA.
+ * per beam; DEDISP_PAIR_PITCH).  It is allocated for one beam when a tree_u8 variant is first selected
+ * (dedisp_plan_create, dedisp_plan_set_variant, dedisp_plan_load_tuning, dedisp_tune, or the first
+ * dedisp_execute_variant of such a variant); this call grows it to nr_beams beams so that dedisp_execute
+ * runs a whole batch in one kernel launch.  Without it a larger batch still works: dedisp_execute then
+ * goes through the workspace as many beams at a time as it holds.
+ * Allocates; does not synchronise; never shrinks.  The block it replaces is kept until
+ * dedisp_plan_destroy, because kernels in flight and CUDA graphs captured from dedisp_execute earlier
+ * still name it: such graphs stay valid (they keep running their old group size), at the price of
+ * the old block's memory.  Reserve before the first capture to avoid that.
+ * Errors: INVALID_ARG, ALLOC, CUDA.
  */
 int dedisp_plan_reserve(dedisp_plan *plan, int nr_beams);
 
@@ -118,9 +125,14 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value);
  * no host<->device copy, no function-attribute call (all of that happened when the variant
  * was selected), so the first call on a fresh plan can already be captured into a CUDA graph.
  * fp32 sums are accumulated in fp32 in ascending channel order.
- * An F32 plan may be executed repeatedly and concurrently on different streams.  A U8 plan may
- * be executed repeatedly, but calls on ONE U8 plan must be ordered with respect to each other
- * (same stream, or events): they share the plan's pair workspace (dedisp_plan_reserve).
+ * A plan may be executed repeatedly and concurrently, from several threads and on different streams.
+ * F32 calls are independent of each other.  The tree_u8 calls on ONE U8 plan share its pair workspace
+ * (dedisp_plan_reserve); the library orders them itself: a call on another stream than the plan's last
+ * one makes its stream wait (cudaStreamWaitEvent, no host synchronisation) for that call's kernels, so
+ * such calls run one after the other on the GPU instead of overlapping, and every result is correct.
+ * One exception: a call made while `stream` is being captured into a CUDA graph neither waits nor is
+ * waited for (an event recorded inside a capture cannot order work outside it); replays of such a graph
+ * must be ordered by the caller against other calls and replays that use the same U8 plan.
  * Errors: INVALID_ARG (null, nr_beams < 1, misaligned base, current device is not the plan's),
  * CUDA (launch error).
  */

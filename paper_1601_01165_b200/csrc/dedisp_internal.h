@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <deque>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -66,12 +67,16 @@ struct TreeInfo {
     bool valid = false;  // every channel's increments are {q_c, q_c + 1}, q_c <= 7
     int qmax = -1;       // max_c q_c
     int *d_qc = nullptr; // device: q_c per channel
-    std::mutex mu;       // guards tables (built when a tree variant is first selected or run)
-    std::vector<TreeTable> tables;
-    const TreeTable *find(int dt, int dms_cta) const {
+    mutable std::mutex mu;  // guards tables (built when a tree variant is first selected or run)
+    std::deque<TreeTable> tables;  // a deque: push_back leaves the entries a launch has looked up in place
+    const TreeTable *find(int dt, int dms_cta) const {   // caller holds mu
         for (const TreeTable &t : tables)
             if (t.dt == dt && t.dms_cta == dms_cta) return &t;
         return nullptr;
+    }
+    const TreeTable *find_locked(int dt, int dms_cta) const {
+        std::lock_guard<std::mutex> lk(mu);
+        return find(dt, dms_cta);
     }
 };
 
@@ -113,39 +118,4 @@ cudaError_t pack_pairs(const uint8_t *d_in, uint32_t *d_pairs, int nr_beams, int
 void set_last_error(const char *what, cudaError_t e);
 void set_last_error_text(const char *msg);  // a message that is not a CUDA error (dedisp_last_error)
 
-// Three-stage host pipeline of dedisp_execute_host_async (host_pipe.cu).
-struct HostPipe {
-    static constexpr int kSlots = 3;
-    bool ready = false;
-    cudaStream_t s_h2d = nullptr, s_exec = nullptr, s_d2h = nullptr;
-    void *in[kSlots] = {}, *out[kSlots] = {};
-    cudaEvent_t ev_in[kSlots] = {}, ev_exec[kSlots] = {}, ev_out[kSlots] = {};
-    size_t in_bytes = 0, out_bytes = 0;
-    uint64_t calls = 0;
-    void destroy();
-};
-
 }  // namespace dedisp
-
-struct dedisp_plan {
-    int C, D, dtype;
-    int64_t S, M;
-    int in_pitch, dpitch;
-    double f_low, bw, rate, dm_first, dm_step;
-    int32_t *d_shift = nullptr;
-    int32_t *d_shiftT = nullptr;
-    std::vector<int32_t> h_shift;  // [D][C]
-    int max_step = 0;
-    std::vector<dedisp::VariantFit> fit;  // per variant
-    dedisp::TreeInfo tree;
-    int variant = 0;
-    int device = 0;                // the CUDA device the plan's tables live on
-    // uint8 tree kernels: the input repacked as pairs of samples S2 apart (pack_pairs_kernel)
-    int S2 = 0, pair_pitch = 0;
-    uint32_t *d_pairs = nullptr;   // [pairs_beams][C][pair_pitch]
-    int pairs_beams = 0;
-    // host-buffer path workspace (dedisp_execute_host)
-    void *ws_in = nullptr, *ws_out = nullptr;
-    size_t ws_in_bytes = 0, ws_out_bytes = 0;
-    dedisp::HostPipe pipe;  // dedisp_execute_host_async
-};

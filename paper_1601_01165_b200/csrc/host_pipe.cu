@@ -5,7 +5,7 @@
 // copy of call n-1 run on three streams over kSlots device workspaces, ordered by events.
 #include <cstdio>
 
-#include "dedisp_internal.h"
+#include "plan_object.h"
 
 using namespace dedisp;
 

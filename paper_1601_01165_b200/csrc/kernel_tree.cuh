@@ -64,6 +64,14 @@ struct TreeTile {
     static_assert(CC <= 32, "one lane per channel of a chunk issues its copies");
     static_assert(DT <= 9 && QMAX <= 7, "8 increment bits and a one-hot q per descriptor");
     static_assert(HALF % AL == 0, "time tiles start on 16-byte boundaries of the staged rows");
+    // uint8: what the 16-bit pair counters and the carry-chain adds of gen_tree.py rely on.  A counter takes
+    // at most 255 per channel and is flushed every FLUSH_CHUNKS chunks, so it cannot carry into its
+    // neighbour; the chains join accumulators k and k + 1, so TT must be even for a chain never to join a
+    // valid element with one past the row's end (plan.cu checks the matching run-time conditions:
+    // S2 a multiple of 4 and pair_pitch >= S2 + M).
+    static_assert(!U8 || FLUSH_CHUNKS * CC * 255 < 65536, "a 16-bit pair counter would overflow between flushes");
+    static_assert(!U8 || FLUSH_CHUNKS >= 1, "at least one chunk between flushes");
+    static_assert(TT % 2 == 0, "carry chains join accumulators k and k + 1");
 };
 
 // Shared memory (dynamic): mbarriers | NSTAGE stages { CC rows of lrow staged elements | (CC + 1) x WD

@@ -9,7 +9,7 @@
 #include <map>
 #include <mutex>
 
-#include "dedisp_internal.h"
+#include "plan_object.h"
 
 namespace dedisp {
 
@@ -128,10 +128,42 @@ static int ensure_tree_table(dedisp_plan *pl, int v) {
     return DEDISP_OK;
 }
 
+// The uint8 tree kernels' pair workspace for nr_beams beams (never shrinks).  An outgrown block is retired,
+// not freed: kernels in flight and CUDA graphs captured earlier may still name it, and calls that follow
+// are ordered behind the last one by the hand-over event anyway (launch_variant), so no synchronisation is
+// needed here.  Retired blocks are freed by dedisp_plan_destroy.
+static int grow_pairs(dedisp_plan *pl, int nr_beams) {
+    std::lock_guard<std::mutex> lk(pl->pairs_mu);
+    if (nr_beams <= pl->pairs_beams) return DEDISP_OK;
+    cudaError_t e;
+    if (!pl->pairs_done && (e = cudaEventCreateWithFlags(&pl->pairs_done, cudaEventDisableTiming)) != cudaSuccess) {
+        set_last_error("cudaEventCreate(pair workspace)", e);
+        return DEDISP_ERR_CUDA;
+    }
+    uint32_t *p = nullptr;
+    e = cudaMalloc(&p, (size_t)nr_beams * pl->C * pl->pair_pitch * 4);
+    if (e != cudaSuccess) {
+        cudaGetLastError();  // the failed allocation must not show up as the next launch's error
+        set_last_error("cudaMalloc(pair workspace)", e);
+        return DEDISP_ERR_ALLOC;
+    }
+    try {
+        if (pl->d_pairs) pl->retired_pairs.push_back(pl->d_pairs);
+    } catch (...) { cudaFree(p); return DEDISP_ERR_ALLOC; }
+    pl->d_pairs = p;
+    pl->pairs_beams = nr_beams;
+    return DEDISP_OK;
+}
+
+static bool needs_pairs(const dedisp_plan *pl, int v) {
+    return pl->dtype == DEDISP_U8 && variants()[v].kind == KIND_TREE;
+}
+
 // Everything a variant needs before its first launch, done when it is SELECTED (plan creation,
 // set_variant, load_tuning, tune) so that dedisp_execute itself neither allocates nor touches
 // function attributes: the large-shared-memory attribute (per device: set unconditionally, it is
-// cheap) and, for tree variants, the descriptor table.
+// cheap), for tree variants the descriptor table, and for uint8 tree variants the pair workspace
+// (one beam, unless dedisp_plan_reserve asked for more): only the variants that run pay for it.
 static int prepare_variant(dedisp_plan *pl, int v) {
     const VariantFit &f = pl->fit[v];
     if (!f.ok) return DEDISP_ERR_INVALID_ARG;
@@ -139,7 +171,9 @@ static int prepare_variant(dedisp_plan *pl, int v) {
         cudaError_t e = variants()[v].prepare(f.smem);
         if (e != cudaSuccess) { set_last_error("cudaFuncSetAttribute", e); return DEDISP_ERR_CUDA; }
     }
-    return ensure_tree_table(pl, v);
+    int rc = ensure_tree_table(pl, v);
+    if (rc == DEDISP_OK && needs_pairs(pl, v)) rc = grow_pairs(pl, 1);
+    return rc;
 }
 
 // Adds per clock and SM the tree tiles sustain on B200 (round-2 measurements on apertif / survey8, tile
@@ -170,7 +204,7 @@ static double tree_rate(bool u8, int dt, int tt, int warps, int cc, int lazy) {
 // shared-memory cap, generic ~10 = 4-byte loads at the L2's per-SM share; tree tiles: tree_rate) and of the bytes it stages
 // from L2 (~40 B/clk/SM); an SM runs ceil(CTAs / 148) of them (wave quantisation), more slowly when
 // too few warps are resident to hide latencies.  dedisp_tune replaces the guess by a measurement.
-static int heuristic_variant(const dedisp_plan *pl) {
+static int heuristic_variant(const dedisp_plan *pl, bool allow_tree = true) {
     const auto &vs = variants();
     double best = 1e300;
     int bi = -1;  // no variant supports the plan: dedisp_plan_create reports it
@@ -178,6 +212,7 @@ static int heuristic_variant(const dedisp_plan *pl) {
     for (size_t v = 0; v < vs.size(); ++v) {
         if (!pl->fit[v].ok) continue;
         const Variant &x = vs[v];
+        if (!allow_tree && x.kind == KIND_TREE) continue;
         const double tile = (double)x.dt * x.tt;
         double rate, need, occ;
         if (x.kind == KIND_TREE) {
@@ -278,6 +313,14 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     // uint8 tree kernels: pair y = samples y and y + S2 of a row (kernel_tree.cuh)
     pl->S2 = (int)((((nr_samples + 1) / 2) + 3) & ~(int64_t)3);
     pl->pair_pitch = (int)((pl->S2 + pl->M + 3) & ~(int64_t)3);
+    // what the uint8 tree kernels' carry-chain adds rely on (kernel_tree.cuh, gen_tree.py): a register pair
+    // (k, k + 1) never straddles the end of the valid pairs, and rows are long enough that what lies past a
+    // tile's valid elements only reaches accumulators that are never stored
+    if (pl->S2 % 4 != 0 || pl->pair_pitch < pl->S2 + pl->M || pl->pair_pitch % 4 != 0) {
+        set_last_error_text("internal: pair layout invariants violated (S2 % 4, pair_pitch >= S2 + M)");
+        status = DEDISP_ERR_INVALID_ARG;
+        goto fail;
+    }
     if (build_tree_slopes(pl) != cudaSuccess) goto cuda_fail;
     compute_fits(pl);
     pl->variant = heuristic_variant(pl);
@@ -290,11 +333,16 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     }
     if (const char *cache = getenv("DEDISP_TUNE_CACHE"))
         if (*cache) dedisp_plan_load_tuning(pl, cache, 1, nullptr);  // missing file / entry: keep the heuristic
-    if (in_dtype == DEDISP_U8 && pl->tree.valid) {
-        status = dedisp_plan_reserve(pl, 1);
-        if (status != DEDISP_OK) goto fail;
-    }
     status = prepare_variant(pl, pl->variant);
+    if (status == DEDISP_ERR_ALLOC && variants()[pl->variant].kind == KIND_TREE) {
+        // no memory for a tree variant's descriptor table or pair workspace: the plan still runs on the
+        // best kernel that needs neither
+        const int v = heuristic_variant(pl, false);
+        if (v >= 0) {
+            pl->variant = v;
+            status = prepare_variant(pl, v);
+        }
+    }
     if (status != DEDISP_OK) goto fail;
     *plan = pl;
     return DEDISP_OK;
@@ -309,17 +357,8 @@ fail:
 
 int dedisp_plan_reserve(dedisp_plan *plan, int nr_beams) {
     if (!plan || nr_beams < 1) return DEDISP_ERR_INVALID_ARG;
-    if (plan->dtype != DEDISP_U8 || !plan->tree.valid || nr_beams <= plan->pairs_beams) return DEDISP_OK;
-    // the old workspace may still be read by kernels in flight
-    cudaError_t e = cudaDeviceSynchronize();
-    if (e != cudaSuccess) { set_last_error("cudaDeviceSynchronize", e); return DEDISP_ERR_CUDA; }
-    uint32_t *p = nullptr;
-    e = cudaMalloc(&p, (size_t)nr_beams * plan->C * plan->pair_pitch * 4);
-    if (e != cudaSuccess) { set_last_error("cudaMalloc(pair workspace)", e); return DEDISP_ERR_ALLOC; }
-    if (plan->d_pairs) cudaFree(plan->d_pairs);
-    plan->d_pairs = p;
-    plan->pairs_beams = nr_beams;
-    return DEDISP_OK;
+    if (plan->dtype != DEDISP_U8 || !plan->tree.valid) return DEDISP_OK;
+    return grow_pairs(plan, nr_beams);
 }
 
 int dedisp_shift_table(const dedisp_plan *plan, int32_t *host_out) {
@@ -361,14 +400,34 @@ static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void
     a.C = plan->C; a.D = plan->D; a.S = (int)plan->S; a.in_pitch = plan->in_pitch;
     a.dpitch = plan->dpitch; a.lrow = f.lrow;
     a.pairs = plan->d_pairs; a.pair_pitch = plan->pair_pitch; a.S2 = plan->S2;
-    const TreeTable *tt = x.kind == KIND_TREE ? plan->tree.find(x.dt, x.dms_cta) : nullptr;
+    const TreeTable *tt = x.kind == KIND_TREE ? plan->tree.find_locked(x.dt, x.dms_cta) : nullptr;
     if (x.kind == KIND_TREE && !tt) return DEDISP_ERR_INVALID_ARG;  // variant was never prepared
     a.desc = tt ? tt->d_desc : nullptr;
     a.descpitch = tt ? tt->pitch : 0;
     // grid.z carries the beams (step a7): at most 65535 per launch; the uint8 tree kernels
     // go through the pair workspace, as many beams at a time as it was reserved for
     const bool paired = x.kind == KIND_TREE && plan->dtype == DEDISP_U8;
-    if (paired && (!plan->d_pairs || plan->pairs_beams < 1)) return DEDISP_ERR_INVALID_ARG;
+    // Paired calls on one plan share its pair workspace.  The whole enqueue happens under the plan's
+    // workspace mutex, and the workspace is handed from stream to stream by an event: a call on another
+    // stream than the last paired call's first makes its stream wait for that call's kernels, so calls on
+    // different streams (or from different threads) never overlap on the workspace, whatever the caller
+    // does.  No host synchronisation.  Not while `st` is being captured: events recorded in a capture
+    // cannot order work outside it, so a captured call neither waits nor records, and replays of the graph
+    // are for the caller to order against other calls on the plan (include/dedisp.h).
+    std::unique_lock<std::mutex> pairs_lock(plan->pairs_mu, std::defer_lock);
+    bool hand_over = false;
+    if (paired) {
+        pairs_lock.lock();
+        if (!plan->d_pairs || plan->pairs_beams < 1) return DEDISP_ERR_INVALID_ARG;
+        a.pairs = plan->d_pairs;
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+        hand_over = cap == cudaStreamCaptureStatusNone;
+        if (hand_over && plan->pairs_used && plan->pairs_stream != st) {
+            cudaError_t e = cudaStreamWaitEvent(st, plan->pairs_done, 0);
+            if (e != cudaSuccess) { set_last_error("cudaStreamWaitEvent(pair workspace)", e); return DEDISP_ERR_CUDA; }
+        }
+    }
     const int group = paired ? std::min(plan->pairs_beams, 65535) : 65535;
     const size_t in_beam = (size_t)plan->C * plan->in_pitch * (plan->dtype == DEDISP_U8 ? 1 : 4);
     const size_t out_beam = (size_t)plan->D * plan->S * 4;
@@ -382,6 +441,12 @@ static int launch_variant(const dedisp_plan *plan, int v, const void *d_in, void
                            plan->pair_pitch, plan->S2, st);
         if (e == cudaSuccess) e = x.launch(a, nb, f.smem, st);
         if (e != cudaSuccess) { set_last_error(x.name, e); return DEDISP_ERR_CUDA; }
+    }
+    if (hand_over) {
+        cudaError_t e = cudaEventRecord(plan->pairs_done, st);
+        if (e != cudaSuccess) { set_last_error("cudaEventRecord(pair workspace)", e); return DEDISP_ERR_CUDA; }
+        plan->pairs_stream = st;
+        plan->pairs_used = true;
     }
     return DEDISP_OK;
 }
@@ -459,6 +524,8 @@ int dedisp_plan_destroy(dedisp_plan *plan) {
     for (auto &t : plan->tree.tables)
         if (t.d_desc) cudaFree(t.d_desc);
     if (plan->d_pairs) cudaFree(plan->d_pairs);
+    for (uint32_t *p : plan->retired_pairs) cudaFree(p);
+    if (plan->pairs_done) cudaEventDestroy(plan->pairs_done);
     if (plan->ws_in) cudaFree(plan->ws_in);
     if (plan->ws_out) cudaFree(plan->ws_out);
     delete plan;

@@ -20,7 +20,7 @@
 #include <cstdio>
 #include <mutex>
 
-#include "dedisp_internal.h"
+#include "plan_object.h"
 
 namespace dedisp {
 
@@ -86,7 +86,7 @@ int dedisp_execute_static_scratch(const dedisp_plan *plan, const void *d_in, voi
                             "use scratch memory; call dedisp_execute, which needs none for this plan");
         return DEDISP_ERR_INVALID_ARG;
     }
-    const TreeTable *tt = plan->tree.find(x.dt, x.dms_cta);
+    const TreeTable *tt = plan->tree.find_locked(x.dt, x.dms_cta);
     if (!tt) return DEDISP_ERR_INVALID_ARG;  // cannot happen for the selected variant: it was prepared
     const size_t beam_words = (size_t)plan->C * (size_t)plan->pair_pitch;
     if (beam_words > kStaticScratchWords) {

@@ -9,7 +9,7 @@
 #include <sstream>
 #include <string>
 
-#include "dedisp_internal.h"
+#include "plan_object.h"
 
 using namespace dedisp;
 

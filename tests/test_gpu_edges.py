@@ -144,7 +144,19 @@ def test_u8_batches_larger_than_the_reserved_workspace(dd):
     plan, table, x, d_in = make_case(dd, s)
     ref = oracle.dedisperse(x, table, s.nr_samples)
     tv = [v for v in plan.supported_variants() if dd.variant_name(v).startswith("tree_u8")]
-    assert tv and plan.reserved_beams == 1
+    lds = [v for v in plan.supported_variants() if dd.variant_name(v).startswith("lds_u8")]
+    assert tv and lds
+    # only the variants that run pay for the workspace: a fresh plan on a tree_u8 kernel holds one beam of
+    # it, a plan on another kernel none until a tree_u8 variant is selected
+    is_tree = dd.variant_name(plan.variant).startswith("tree_u8")
+    assert plan.reserved_beams == (1 if is_tree else 0)
+    with dd.Plan(*s.plan_args()) as other:
+        other.set_variant(lds[0])
+        held = other.reserved_beams
+        other.set_variant(tv[0])
+        assert held in (0, 1) and other.reserved_beams == 1 and other.pair_pitch > s.nr_samples // 2
+    plan.set_variant(tv[0])
+    assert plan.reserved_beams == 1
     for resv in (1, 2, 5):
         plan.reserve(resv)
         assert plan.reserved_beams == max(resv, 1)
