@@ -86,22 +86,23 @@ def compulsory_bytes(s, in_samples):
     return s.nr_beams * (s.nr_channels * in_samples * esz + s.nr_dms * s.nr_samples * 4)
 
 
-def binding_roof(vname, s, sm_max_mhz):
+def binding_roof(vname, s, sm_max_mhz, sm_count=SM_COUNT):
     """The on-chip roof that bounds the variant's kind of kernel, in T adds/s
-    at the maximum SM clock: (bound, peak, note)."""
+    at the maximum SM clock: (bound, peak, note).  sm_count: the device's SM count (run_ours reads it from the
+    device; 148 on a B200)."""
     clk = sm_max_mhz * 1e6
     if vname.startswith("tree_u8"):
-        return ("alu", SM_COUNT * INT_LANES_PER_SM * 2 * clk / 1e12,
-                "packed 16-bit adds: 148 SMs x 128 integer-add lanes (64 IADD3 + 64 IMAD) x 2 counters "
-                "per 32-bit add x %.0f MHz; a pure add stream measures 115 of the 128 lanes" % sm_max_mhz)
+        return ("alu", sm_count * INT_LANES_PER_SM * 2 * clk / 1e12,
+                "packed 16-bit adds: %d SMs x 128 integer-add lanes (64 IADD3 + 64 IMAD) x 2 counters "
+                "per 32-bit add x %.0f MHz; a pure add stream measures 115 of the 128 lanes" % (sm_count, sm_max_mhz))
     if vname.startswith("tree_"):
-        return ("alu", SM_COUNT * FP32_LANES_PER_SM * clk / 1e12,
-                "fp32 adds: 148 SMs x 128 lanes x %.0f MHz max SM clock" % sm_max_mhz)
+        return ("alu", sm_count * FP32_LANES_PER_SM * clk / 1e12,
+                "fp32 adds: %d SMs x 128 lanes x %.0f MHz max SM clock" % (sm_count, sm_max_mhz))
     if vname.startswith("lds_"):
-        return ("lds", SM_COUNT * LDS_WORDS_PER_SM * clk / 1e12,
-                "one shared-memory word per add: 148 SMs x 32 words/clk x %.0f MHz (shared-memory "
-                "wavefronts, not an ALU pipe, bind this kind: profiles/r02_ncu_lds_lofar.md)" % sm_max_mhz)
-    return ("l2", SM_COUNT * 10 * clk / 1e12,
+        return ("lds", sm_count * LDS_WORDS_PER_SM * clk / 1e12,
+                "one shared-memory word per add: %d SMs x 32 words/clk x %.0f MHz (shared-memory "
+                "wavefronts, not an ALU pipe, bind this kind: profiles/r02_ncu_lds_lofar.md)" % (sm_count, sm_max_mhz))
+    return ("l2", sm_count * 10 * clk / 1e12,
             "no-reuse kernel: about 10 four-byte L2 loads per clk and SM (measured, DESIGN.md section 8)")
 
 
@@ -334,7 +335,7 @@ def time_device(case, steps, warmup, barrier, min_warm_s=0.0):
     return ev[0].elapsed_time(ev[-1]), sorted(ev[k].elapsed_time(ev[k + 1]) for k in range(steps))
 
 
-def report(case, world, total_ms, per, steps, hbm_gbs, sm_max_mhz, peak_kind):
+def report(case, world, total_ms, per, steps, hbm_gbs, sm_max_mhz, peak_kind, sm_count=SM_COUNT):
     """The per-config numbers the north star asks for."""
     s = case.s
     B, C, D, S = s.nr_beams, s.nr_channels, s.nr_dms, s.nr_samples
@@ -342,7 +343,7 @@ def report(case, world, total_ms, per, steps, hbm_gbs, sm_max_mhz, peak_kind):
     adds = B * D * C * S
     kern_ms = float(np.mean(per))
     comp = compulsory_bytes(s, case.in_samples)
-    bound, peak, note = binding_roof(case.vname, s, sm_max_mhz)
+    bound, peak, note = binding_roof(case.vname, s, sm_max_mhz, sm_count)
     achieved = adds / (kern_ms * 1e-3) / 1e12
     traffic, src = ncu_traffic(s.name, case.vname)
     rt = (S / s.sample_rate) / (ms_step * 1e-3 / B)
@@ -381,6 +382,7 @@ def run_ours(args, s):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     build.build()
     hbm_gbs, sm_max_mhz, peak_kind = measured_peaks()
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     warmup = max(args.warmup, 3)
 
     def barrier():
@@ -395,7 +397,7 @@ def run_ours(args, s):
     total_ms, per = time_device(case, args.steps, warmup, barrier, min_warm_s=0.6)
     clocks = sampler.stop() if sampler else None
     total_ms = max_over_ranks(total_ms, world)
-    head = report(case, world, total_ms, per, args.steps, hbm_gbs, sm_max_mhz, peak_kind)
+    head = report(case, world, total_ms, per, args.steps, hbm_gbs, sm_max_mhz, peak_kind, sm_count)
 
     # ---- end to end through the host-buffer entry point (pinned host memory): every step uploads
     # its input, runs the kernels and downloads its result; consecutive steps overlap on the library's
@@ -440,20 +442,24 @@ def run_ours(args, s):
     # factor and beams in real time); fewer steps for the long ones
     others = {}
     if not args.only and args.variant is None:
-        for name in wl.CONFIGS:
+        for name in wl.ALL:     # the BASELINE.json configs, then the paper's own two setups
             if name == s.name:
                 continue
-            o = wl.CONFIGS[name]
+            o = wl.ALL[name]
             # a config that cannot run here (e.g. batch40's 11 GB on a smaller device) is reported as
             # such; the headline line is printed either way (single rank only: with replicas every
             # rank must reach the same collectives)
             try:
                 c = Case(o, rank, tune=args.tune)
                 ksteps = args.steps if o.nr_beams == 1 else max(3, args.steps // 4)
-                t_ms, p = time_device(c, ksteps, 3, barrier)
+                # every config gets its own clock record, sampled over its own warm-up and timed steps
+                smp = ClockSampler(local) if rank == 0 else None
+                t_ms, p = time_device(c, ksteps, 3, barrier, min_warm_s=0.4)
+                clk_o = smp.stop() if smp else None
                 t_ms = max_over_ranks(t_ms, world)
-                others[name] = report(c, world, t_ms, p, ksteps, hbm_gbs, sm_max_mhz, peak_kind)
+                others[name] = report(c, world, t_ms, p, ksteps, hbm_gbs, sm_max_mhz, peak_kind, sm_count)
                 others[name]["steps"] = ksteps
+                others[name]["clocks"] = clk_o
                 c.close()
             except Exception as e:  # noqa: BLE001
                 if world > 1:
@@ -493,13 +499,13 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="apertif", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--config", default="apertif", choices=sorted(wl.ALL))
     ap.add_argument("--only", action="store_true", help="time the named config only")
     ap.add_argument("--variant", type=int, default=None, help="force a kernel variant index (implies --only)")
     ap.add_argument("--tune", action="store_true", help="run dedisp_tune before timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    s = wl.CONFIGS[args.config]
+    s = wl.ALL[args.config]
     if args.impl == "reference":
         run_reference(args, s)
     else:

@@ -202,7 +202,7 @@ static double tree_rate(bool u8, int dt, int tt, int warps, int cc, int lazy) {
 // Untuned default: a cost model in SM clocks.  A CTA costs the larger of its adds at the kind's
 // measured rate (adds/clk/SM on B200: tree ~58 for large thread tiles, lds ~28 = the one-word-per-add
 // shared-memory cap, generic ~10 = 4-byte loads at the L2's per-SM share; tree tiles: tree_rate) and of the bytes it stages
-// from L2 (~40 B/clk/SM); an SM runs ceil(CTAs / 148) of them (wave quantisation), more slowly when
+// from L2 (~40 B/clk/SM); an SM runs ceil(CTAs / SM count of the plan's device) of them (wave quantisation), more slowly when
 // too few warps are resident to hide latencies.  dedisp_tune replaces the guess by a measurement.
 static int heuristic_variant(const dedisp_plan *pl, bool allow_tree = true) {
     const auto &vs = variants();
@@ -233,7 +233,7 @@ static int heuristic_variant(const dedisp_plan *pl, bool allow_tree = true) {
         const double adds_cta = (double)x.dms_cta * x.samples_cta * pl->C;
         const double bytes_cta = x.kind == KIND_GENERIC ? 0 : (double)pl->C * (x.samples_cta + pl->fit[v].span) * esz;
         const double t_cta = std::max(adds_cta / rate, bytes_cta / 40.0);
-        const double n_sm = std::ceil(nd * nt / 148.0);
+        const double n_sm = std::ceil(nd * nt / (double)pl->sm_count);
         const double resident = std::min(occ, n_sm);
         const double warp_eff = std::min(1.0, resident * x.threads / 32.0 / need);
         const double cost = n_sm * t_cta / warp_eff + 6000;  // + launch
@@ -284,6 +284,9 @@ int dedisp_plan_create(dedisp_plan **plan, int nr_channels, double f_low_MHz,
     int64_t in_samples;
 
     CUDA_TRY(cudaGetDevice(&pl->device), "cudaGetDevice");
+    CUDA_TRY(cudaDeviceGetAttribute(&pl->sm_count, cudaDevAttrMultiProcessorCount, pl->device),
+             "cudaDeviceGetAttribute(SM count)");
+    if (pl->sm_count < 1) pl->sm_count = 1;
     CUDA_TRY(cudaMalloc(&pl->d_shift, (size_t)nr_dms * nr_channels * 4), "cudaMalloc(shift)");
     CUDA_TRY(cudaMalloc(&pl->d_shiftT, (size_t)nr_channels * pl->dpitch * 4), "cudaMalloc(shiftT)");
     CUDA_TRY(cudaMalloc(&d_flag, 4), "cudaMalloc(flag)");

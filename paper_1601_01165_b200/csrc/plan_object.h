@@ -34,6 +34,7 @@ struct dedisp_plan {
     dedisp::TreeInfo tree;
     int variant = 0;
     int device = 0;                // the CUDA device the plan's tables live on
+    int sm_count = 148;            // its SM count (the untuned default's wave quantisation)
     // uint8 tree kernels: the input repacked as pairs of samples S2 apart (pack_pairs_kernel)
     int S2 = 0, pair_pitch = 0;
     // The workspace is allocated when a tree_u8 variant is first selected (or by dedisp_plan_reserve) and

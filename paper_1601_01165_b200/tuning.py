@@ -1,7 +1,7 @@
 """Shipped tuning results (step a8): winners of dedisp_tune on a B200, one text line per
 (GPU, setup), in the format dedisp_tune appends.  `python -m paper_1601_01165_b200.tuning`
-re-tunes the five BASELINE.json configs (or the ones named on the command line, keeping the other
-entries) on the current GPU and rewrites the file."""
+re-tunes the five BASELINE.json configs and the paper's two setups (or the ones named on the command
+line, keeping the other entries) on the current GPU and rewrites the file."""
 from __future__ import annotations
 
 import os
@@ -30,12 +30,12 @@ def retune(names=None, out_path: str = SHIPPED, beams_cap: int = 8) -> None:
     import torch
 
     from . import dedisp, workloads as wl
-    names = names or list(wl.CONFIGS)
+    names = names or list(wl.ALL)
     tmp = out_path + ".new"
     if os.path.exists(tmp):
         os.remove(tmp)
     for name in names:
-        s = wl.CONFIGS[name]
+        s = wl.ALL[name]
         plan = dedisp.Plan(*s.plan_args())
         nb = min(s.nr_beams, beams_cap)
         in_dt = torch.uint8 if s.in_dtype == wl.U8 else torch.float32

@@ -74,6 +74,18 @@ BATCH40 = replace(APERTIF, name="batch40", nr_beams=40, seed=160101170)
 
 CONFIGS = {s.name: s for s in (TINY, APERTIF, LOFAR, SURVEY8, BATCH40)}
 
+# The paper's own two setups at their largest instance (Table 2 and the 12 input
+# instances of 2-4096 DMs: "DMs from 0, step 0.25" for both).  Apertif: 20 kHz sampling, 300 MHz in 1024
+# channels above 1420 MHz, 4096 DMs.  LOFAR: 200 kHz sampling, 6 MHz in 32 channels above 138 MHz; 2048 DMs
+# is the largest instance whose input row (S + M = 0.2 M + 1.82 M samples) is still a few hundred MB.
+# SURVEY.md 8(f) row 2; not BASELINE.json configs, so they are kept apart from CONFIGS.
+APERTIF_PAPER = Setup("apertif_paper", 1024, 1420.0, 300.0 / 1024, 20000.0, 20000, 0.0, 0.25, 4096,
+                      seed=160101171)
+LOFAR_PAPER = Setup("lofar_paper", 32, 138.0, 6.0 / 32, 200000.0, 200000, 0.0, 0.25, 2048,
+                    seed=160101172)
+PAPER_SETUPS = {s.name: s for s in (APERTIF_PAPER, LOFAR_PAPER)}
+ALL = {**CONFIGS, **PAPER_SETUPS}
+
 
 def scaled(setup: Setup, **kw) -> Setup:
     """A smaller/larger variant of a setup (same band and DM grid unless overridden)."""

@@ -67,5 +67,5 @@ def test_partial_retune_keeps_the_other_entries():
     assert tuning.merge_entries(old, new) == "k1\tvariant a\t1 ms\nk2\tvariant c\t1.5 ms\nk3\tvariant d\t3 ms\n"
     assert tuning.merge_entries("", new) == new
     shipped = open(tuning.SHIPPED).read()
-    assert tuning.merge_entries(shipped, "") == shipped       # five entries, unique keys
-    assert len({l.split("\t")[0] for l in shipped.splitlines()}) == 5
+    assert tuning.merge_entries(shipped, "") == shipped       # unique keys: the five BASELINE configs (apertif
+    assert len({l.split("\t")[0] for l in shipped.splitlines()}) == 7   # for 1 and 8 beams) + the paper's two setups

@@ -169,6 +169,42 @@ def _oracle_blocks(x, table, setup, rows_per_block):
         yield lo, hi, ref, sabs
 
 
+@pytest.mark.parametrize("name", ["apertif_paper", "lofar_paper"])
+def test_paper_setups_full_size_every_output(dd, name):
+    """The paper's own setups (Table 2, DM step 0.25) at their largest instance, EVERY output
+    against the oracle in DM-row blocks: 82 M outputs / 84 G adds (Apertif, 4096 DMs) and 410 M outputs / 13 G
+    adds (LOFAR, 2048 DMs, max shift 1.82 M samples, input rows of 2.02 M samples).  Checked on the kernel
+    dedisp_execute launches (shipped winner) and, for the LOFAR setup, on every staged variant that supports
+    it: the long-span lds tiles this band needs (shift steps of up to ~900 samples per DM) and the generic
+    kernel as the independent third."""
+    torch = _torch()
+    from paper_1601_01165_b200 import tuning
+    s = wl.PAPER_SETUPS[name]
+    plan, table, x, d_in = make_case(dd, s)
+    tuning.apply_shipped(plan)
+    todo = [plan.variant]
+    if name == "lofar_paper":
+        other = [v for v in plan.supported_variants() if v != plan.variant]
+        lds = [v for v in other if dd.variant_name(v).startswith("lds_f32")]
+        todo += lds[:4] + [v for v in other if dd.variant_name(v).startswith("generic")]   # 1.6 GB of host memory each
+    gots = []
+    for v in todo:
+        d_out = out_buffer(s, fill=float("nan"))
+        plan.execute_variant(v, d_in, d_out)
+        torch.cuda.synchronize()
+        gots.append(to_host(s, d_out))
+        del d_out
+    assert len(todo) == 1 or any(dd.variant_name(v).startswith("lds_f32") for v in todo)
+    for lo, hi, ref, sabs in _oracle_blocks(x, table, s, 256):
+        lim = TOL * sabs
+        for v, got in zip(todo, gots):
+            ok = np.abs(got[:, lo:hi] - ref) <= lim      # NaN (an output never written) fails this
+            assert ok.all(), "%s, DM rows %d..%d: %d outputs out of tolerance" % (
+                dd.variant_name(v), lo, hi, (~ok).sum())
+    assert int(table.max()) + s.nr_samples == plan.in_samples
+    plan.destroy()
+
+
 @pytest.mark.parametrize("name", ["apertif", "lofar", "survey8"])
 def test_full_size_every_output(dd, name):
     """BASELINE.json sizes in the launch configuration bench.py times (plan default after
