@@ -57,6 +57,7 @@ enum {
     DEDISP_IN_DTYPE = 8,
     DEDISP_MAX_STEP = 9,   /* max over (c, i) of shift(c, i+1) - shift(c, i) */
     DEDISP_RESERVED_BEAMS = 10, /* U8 plans: beams the pair workspace holds (dedisp_plan_reserve); else 0 */
+    DEDISP_STREAM_H2D_BYTES = 12, /* bytes the last dedisp_stream_block_async call uploaded (0 before the first) */
     DEDISP_PAIR_PITCH = 11 /* U8 plans: 4-byte pairs per row of the pair workspace (nr_samples / 2 rounded up
                               to 4, plus MAX_SHIFT, rounded up to 4): one beam of workspace or static scratch
                               takes nr_channels * PAIR_PITCH * 4 bytes; else 0 */
@@ -224,16 +225,27 @@ int dedisp_host_sync(dedisp_plan *plan);
  * dedisp_stream_block_async -- streaming operation on one beam's long time series (SURVEY.md 8(f)
  * row 4; the paper's real-time setting): dedisperse the block of nr_samples output
  * samples that starts at sample t0, through the same pipeline as dedisp_execute_host_async.
- *   h_series: HOST, [nr_channels][series_pitch] elements; columns [t0, t0 + S + M) of every row are
- *             read, so consecutive blocks (t0 += S) share their last / first M input samples: nothing
- *             is carried over on the device.
+ *   h_series: HOST, [nr_channels][series_pitch] elements; the block needs columns [t0, t0 + S + M) of every row.
  *   h_out   : HOST, [nr_dms][out_pitch] of float / uint32_t; columns [t0, t0 + S) of every row are
  *             written: out[i][t] = sum_c series[c][t + shift(c, dm_i)] for t in the block.
  * Both page-locked and valid until dedisp_host_sync.  The copies are strided (2-D) DMA transfers.
+ * Carry-over: consecutive blocks share M input samples per channel.  When a call continues the plan's
+ * previous call (same h_series and series_pitch, t0 = previous t0 + S), the shared columns
+ * [t0, t0 + M) are NOT uploaded again: they are moved on the device from the previous block's rows, and
+ * only the S new columns [t0 + M, t0 + S + M) of every row cross the bus (nr_channels * S elements per
+ * block instead of nr_channels * (S + M): 10x fewer for the paper's LOFAR setup, where M = 9 S).  The
+ * first block, a block that does not continue the previous one, and the block after dedisp_stream_reset,
+ * dedisp_execute_host_async or a workspace growth upload all S + M columns.  Consequence: a change the
+ * host makes to columns it has already streamed is not seen by the next block unless dedisp_stream_reset
+ * is called first.  dedisp_plan_get(DEDISP_STREAM_H2D_BYTES) tells what the last call uploaded.
  * Errors: INVALID_ARG (null, t0 < 0, series_pitch < t0 + S + M, out_pitch < t0 + S), ALLOC, CUDA.
  */
 int dedisp_stream_block_async(dedisp_plan *plan, const void *h_series, int64_t series_pitch,
                               void *h_out, int64_t out_pitch, int64_t t0);
+
+/* dedisp_stream_reset -- forget what the last stream block left on the device: the next
+ * dedisp_stream_block_async uploads all S + M columns of its rows.  Enqueues nothing.  Errors: INVALID_ARG. */
+int dedisp_stream_reset(dedisp_plan *plan);
 
 /* dedisp_plan_destroy -- frees the plan's host and device tables.  NULL is a no-op. */
 int dedisp_plan_destroy(dedisp_plan *plan);
@@ -259,7 +271,10 @@ int dedisp_plan_set_variant(dedisp_plan *plan, int variant);
  * dedisp_tune -- exhaustive sweep in the spirit of PAPER.md:76 ("try all meaningful
  * combinations and select the best performing one"): times every supported variant on the
  * caller's buffers (same contract as dedisp_execute; d_out is overwritten) with CUDA events
- * on `stream` (synchronises), selects the fastest, and, if cache_path != NULL, persists
+ * on `stream` (synchronises; every variant runs back to back on the one buffer pair the caller gives, so
+ * inputs smaller than the 126 MB L2 are timed L2-warm: the kernels are bound on chip, which keeps the
+ * ranking, but the absolute times are up to a few per cent below bench.py's, which rotates buffer sets),
+ * selects the fastest, and, if cache_path != NULL, persists
  * the winner (one text line "key<TAB>variant name<TAB>note", appended; the last matching line
  * wins on load).  The key is GPU name + setup + a batch-size class (1 beam / 2-7 / 8 or more:
  * the best tile differs when one beam leaves the last wave of CTAs part empty).  ms_out (host, may be NULL)

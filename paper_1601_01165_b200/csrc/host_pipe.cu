@@ -30,6 +30,7 @@ void HostPipe::destroy() {
     s_h2d = s_exec = s_d2h = nullptr;
     in_bytes = out_bytes = 0;
     ready = false;
+    st_valid = false;
 }
 
 // Streams and events once; workspaces grown (after draining the pipeline) when a call needs more.
@@ -77,6 +78,7 @@ static int pipe_prepare(HostPipe &p, size_t in_bytes, size_t out_bytes) {
         }
         if (in_bytes > p.in_bytes) p.in_bytes = in_bytes;
         if (out_bytes > p.out_bytes) p.out_bytes = out_bytes;
+        p.st_valid = false;  // the workspaces that held the last block are gone
     }
     return DEDISP_OK;
 }
@@ -125,13 +127,33 @@ static int pipe_call(dedisp_plan *plan, const void *h_in, void *h_out, int nr_be
     const bool reused = p.calls >= (uint64_t)HostPipe::kSlots;
     // stage 1: H2D into slot s once the kernel that last read this slot's input has finished
     if (reused) PIPE_TRY(cudaStreamWaitEvent(p.s_h2d, p.ev_exec[s], 0), "cudaStreamWaitEvent");
-    if (series_pitch == 0)
+    if (series_pitch == 0) {
+        p.st_valid = false;
         PIPE_TRY(cudaMemcpyAsync(p.in[s], h_in, in_bytes, cudaMemcpyHostToDevice, p.s_h2d), "H2D");
-    else
-        PIPE_TRY(cudaMemcpy2DAsync(p.in[s], (size_t)plan->in_pitch * esz,
-                                   (const char *)h_in + (size_t)t0 * esz, (size_t)series_pitch * esz,
-                                   (size_t)(plan->S + plan->M) * esz, (size_t)plan->C,
-                                   cudaMemcpyHostToDevice, p.s_h2d), "H2D (2-D)");
+    } else {
+        // Carry-over ("the last M input samples carried over"): if this block follows
+        // the previous call's block in time on the same series, its input columns [t0, t0 + M) are the
+        // columns [S, S + M) of the rows the previous call uploaded, which still sit in that call's slot.
+        // They are moved device to device (on the upload stream, which ran that upload itself, so stream
+        // order is enough), and only the S new columns of every row cross the bus.
+        const bool carry = p.st_valid && p.st_series == h_in && p.st_pitch == series_pitch &&
+                           p.st_next_t0 == t0 && p.calls > 0;
+        p.st_valid = false;  // until this call has enqueued all of its copies
+        const size_t row_bytes = (size_t)plan->in_pitch * esz;
+        size_t skip = 0;     // leading columns of every row that do not come from the host
+        if (carry && plan->M > 0) {
+            const int prev = (int)((p.calls - 1) % HostPipe::kSlots);
+            skip = (size_t)plan->M;
+            PIPE_TRY_DRAIN(cudaMemcpy2DAsync(p.in[s], row_bytes, (const char *)p.in[prev] + (size_t)plan->S * esz,
+                                             row_bytes, skip * esz, (size_t)plan->C, cudaMemcpyDeviceToDevice,
+                                             p.s_h2d), "carry-over (D2D, 2-D)");
+        }
+        PIPE_TRY_DRAIN(cudaMemcpy2DAsync((char *)p.in[s] + skip * esz, row_bytes,
+                                         (const char *)h_in + ((size_t)t0 + skip) * esz, (size_t)series_pitch * esz,
+                                         ((size_t)(plan->S + plan->M) - skip) * esz, (size_t)plan->C,
+                                         cudaMemcpyHostToDevice, p.s_h2d), "H2D (2-D)");
+        p.st_h2d_bytes = (int64_t)(((size_t)(plan->S + plan->M) - skip) * esz * (size_t)plan->C);
+    }
     PIPE_TRY_DRAIN(cudaEventRecord(p.ev_in[s], p.s_h2d), "cudaEventRecord");
     // stage 2: the kernels, once the input is there and the slot's previous output has left
     PIPE_TRY_DRAIN(cudaStreamWaitEvent(p.s_exec, p.ev_in[s], 0), "cudaStreamWaitEvent");
@@ -149,6 +171,12 @@ static int pipe_call(dedisp_plan *plan, const void *h_in, void *h_out, int nr_be
                                    cudaMemcpyDeviceToHost, p.s_d2h), "D2H (2-D)");
     PIPE_TRY_DRAIN(cudaEventRecord(p.ev_out[s], p.s_d2h), "cudaEventRecord");
     ++p.calls;
+    if (series_pitch != 0) {
+        p.st_valid = true;
+        p.st_series = h_in;
+        p.st_pitch = series_pitch;
+        p.st_next_t0 = t0 + plan->S;
+    }
     return DEDISP_OK;
 }
 
@@ -165,6 +193,12 @@ extern "C" int dedisp_stream_block_async(dedisp_plan *plan, const void *h_series
         out_pitch < t0 + plan->S)
         return DEDISP_ERR_INVALID_ARG;
     return pipe_call(plan, h_series, h_out, 1, series_pitch, out_pitch, t0);
+}
+
+extern "C" int dedisp_stream_reset(dedisp_plan *plan) {
+    if (!plan) return DEDISP_ERR_INVALID_ARG;
+    plan->pipe.st_valid = false;
+    return DEDISP_OK;
 }
 
 extern "C" int dedisp_host_sync(dedisp_plan *plan) {

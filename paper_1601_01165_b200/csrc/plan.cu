@@ -388,6 +388,7 @@ int dedisp_plan_get(const dedisp_plan *plan, int what, int64_t *value) {
         case DEDISP_MAX_STEP: *value = plan->max_step; break;
         case DEDISP_RESERVED_BEAMS: *value = plan->dtype == DEDISP_U8 ? plan->pairs_beams : 0; break;
         case DEDISP_PAIR_PITCH: *value = plan->dtype == DEDISP_U8 ? plan->pair_pitch : 0; break;
+        case DEDISP_STREAM_H2D_BYTES: *value = plan->pipe.st_h2d_bytes; break;
         default: return DEDISP_ERR_INVALID_ARG;
     }
     return DEDISP_OK;

@@ -16,6 +16,12 @@ struct HostPipe {
     cudaEvent_t ev_in[kSlots] = {}, ev_exec[kSlots] = {}, ev_out[kSlots] = {};
     size_t in_bytes = 0, out_bytes = 0;
     uint64_t calls = 0;
+    // streaming (dedisp_stream_block_async): what the LAST call left on the device, so that the block that
+    // follows it in time takes its first M input columns from there instead of uploading them again
+    bool st_valid = false;          // the last call was a stream block and its slot still holds its input
+    const void *st_series = nullptr;
+    int64_t st_pitch = 0, st_next_t0 = 0;
+    int64_t st_h2d_bytes = 0;       // host-to-device bytes of the last stream block (DEDISP_STREAM_H2D_BYTES)
     void destroy();
 };
 

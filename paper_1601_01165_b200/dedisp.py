@@ -18,13 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
 
 F32, U8 = 0, 1
 (MAX_SHIFT, IN_SAMPLES, IN_PITCH, OUT_PITCH, VARIANT, NR_CHANNELS, NR_DMS, NR_SAMPLES, IN_DTYPE,
- MAX_STEP, RESERVED_BEAMS, PAIR_PITCH) = range(12)
+ MAX_STEP, RESERVED_BEAMS, PAIR_PITCH, STREAM_H2D_BYTES) = range(13)
 
 # every symbol include/dedisp.h declares
 SYMBOLS = [
     "dedisp_plan_create", "dedisp_plan_reserve", "dedisp_shift_table", "dedisp_plan_get", "dedisp_execute",
     "dedisp_execute_variant", "dedisp_execute_static_scratch", "dedisp_static_scratch_bytes", "dedisp_execute_host", "dedisp_execute_host_async", "dedisp_host_sync",
-    "dedisp_stream_block_async",
+    "dedisp_stream_block_async", "dedisp_stream_reset",
     "dedisp_plan_destroy", "dedisp_variant_count",
     "dedisp_variant_name", "dedisp_variant_supported", "dedisp_plan_set_variant", "dedisp_tune",
     "dedisp_plan_load_tuning", "dedisp_status_string", "dedisp_last_error",
@@ -62,6 +62,7 @@ def load_library() -> ctypes.CDLL:
     lib.dedisp_execute_host_async.argtypes = [vp, vp, vp, ci]
     lib.dedisp_host_sync.argtypes = [vp]
     lib.dedisp_stream_block_async.argtypes = [vp, vp, i64, vp, i64, i64]
+    lib.dedisp_stream_reset.argtypes = [vp]
     lib.dedisp_plan_destroy.argtypes = [vp]
     lib.dedisp_variant_count.argtypes = []
     lib.dedisp_variant_name.argtypes = [ci]
@@ -165,6 +166,7 @@ class Plan:
     max_step = property(lambda self: self.get(MAX_STEP))
     reserved_beams = property(lambda self: self.get(RESERVED_BEAMS))
     pair_pitch = property(lambda self: self.get(PAIR_PITCH))
+    stream_h2d_bytes = property(lambda self: self.get(STREAM_H2D_BYTES))
 
     def reserve(self, nr_beams: int):
         """dedisp_plan_reserve: size the uint8 pair workspace for batches of nr_beams beams."""
@@ -210,6 +212,10 @@ class Plan:
         _check(self._lib.dedisp_stream_block_async(self._h, _addr(h_series), int(series_pitch),
                                                    _addr(h_out), int(out_pitch), int(t0)),
                "dedisp_stream_block_async")
+
+    def stream_reset(self):
+        """dedisp_stream_reset: the next stream block uploads all of its S + M input columns again."""
+        _check(self._lib.dedisp_stream_reset(self._h), "dedisp_stream_reset")
 
     def host_sync(self):
         _check(self._lib.dedisp_host_sync(self._h), "dedisp_host_sync")

@@ -97,9 +97,10 @@ def stream(nblocks: int = 12):
     import torch
 
     from . import tuning
-    print("| setup | blocks | ms per 1-s block, end to end | seconds of data per second | host<->device GB/s |")
-    print("|---|---|---|---|---|")
-    for s in (wl.APERTIF, wl.SURVEY8):
+    print("| setup | blocks | ms per block, end to end | seconds of data per second | MB uploaded per block "
+          "(first block) | host<->device GB/s |")
+    print("|---|---|---|---|---|---|")
+    for s in (wl.APERTIF, wl.SURVEY8, wl.LOFAR_PAPER):
         plan = dedisp.Plan(*s.plan_args())
         tuning.apply_shipped(plan)
         S, M = s.nr_samples, plan.max_shift
@@ -110,14 +111,21 @@ def stream(nblocks: int = 12):
         for b in range(3):   # warm-up: workspaces, kernel attributes
             plan.stream_block_async(h_series, total + M, h_out, total, b * S)
         plan.host_sync()
+        plan.stream_reset()
+        plan.stream_block_async(h_series, total + M, h_out, total, 0)
+        first = plan.stream_h2d_bytes
+        plan.stream_block_async(h_series, total + M, h_out, total, S)
+        later = plan.stream_h2d_bytes
+        plan.host_sync()
+        plan.stream_reset()
         t0 = time.perf_counter()
         for b in range(nblocks):
             plan.stream_block_async(h_series, total + M, h_out, total, b * S)
         plan.host_sync()
         dt = (time.perf_counter() - t0) / nblocks
-        nbytes = s.nr_channels * (S + M) * h_series.element_size() + s.nr_dms * S * 4
-        print("| %s | %d | %.2f | %.0f | %.1f |" % (s.name, nblocks, dt * 1e3, s.seconds_of_data / dt,
-                                                    nbytes / dt / 1e9), flush=True)
+        nbytes = later + s.nr_dms * S * 4
+        print("| %s | %d | %.2f | %.0f | %.1f (%.1f) | %.1f |" % (s.name, nblocks, dt * 1e3, s.seconds_of_data / dt,
+                                                                later / 1e6, first / 1e6, nbytes / dt / 1e9), flush=True)
         plan.destroy()
         del h_series, h_out
 

@@ -242,8 +242,12 @@ def test_streaming_blocks_equal_one_long_dedispersion(dd, u8):
     ref = oracle.dedisperse(series[None], table, total)[0]
     h_series = torch.from_numpy(series).pin_memory()
     h_out = torch.full((s.nr_dms, total + 3), -1, dtype=torch.int32 if u8 else torch.float32).pin_memory()
+    esz = 1 if u8 else 4
     for b in range(nblk):
         plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, b * S)
+        # the first block uploads S + M columns per row, every later one only its S new columns: the M
+        # shared ones are carried over on the device
+        assert plan.stream_h2d_bytes == s.nr_channels * (S + (M if b == 0 else 0)) * esz
     plan.host_sync()
     got = h_out.numpy()[:, :total]
     if u8:
@@ -251,8 +255,46 @@ def test_streaming_blocks_equal_one_long_dedispersion(dd, u8):
     else:
         assert np.array_equal(got.astype(np.float64), ref)
     assert (h_out.numpy()[:, total:] == -1).all()     # nothing written past the blocks
+    # a block that does not continue the last one, and the block after a reset, upload everything; the
+    # results are the same bits
+    h_out.fill_(-1)
+    for b, full in ((3, True), (4, False), (2, True), (3, False)):
+        plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, b * S)
+        assert plan.stream_h2d_bytes == s.nr_channels * (S + (M if full else 0)) * esz
+    plan.stream_reset()
+    plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, 4 * S)
+    assert plan.stream_h2d_bytes == s.nr_channels * (S + M) * esz
+    plan.host_sync()
+    got = h_out.numpy()[:, 2 * S:5 * S]
+    assert np.array_equal(got.view(np.uint32).astype(np.uint64) if u8 else got.astype(np.float64), ref[:, 2 * S:5 * S])
     with pytest.raises(dd.DedispError):
         plan.stream_block_async(h_series, series.shape[1], h_out, total + 3, total)  # past the end
+    plan.destroy()
+
+
+def test_streaming_with_shifts_longer_than_the_block_carries_them_over(dd):
+    """The paper's LOFAR band at DM step 0.25: the max shift M is several times the block length
+    S, so M of the S + M input columns of every block are already on the device.  8 consecutive blocks equal one
+    long oracle run within the fp32 tolerance (Gaussian data), and every block after the first uploads
+    nr_channels * S elements."""
+    import torch
+    S, nblk = 6000, 8
+    s = wl.scaled(wl.LOFAR_PAPER, name="stream_long", nr_dms=64, nr_samples=S)
+    plan = dd.Plan(*s.plan_args())
+    table = oracle.shift_table(*s.table_args())
+    M = plan.max_shift
+    assert M >= 5 * S
+    total = nblk * S
+    series = wl.make_input(wl.scaled(s, nr_samples=total), total + M, total + M + 1)[0]
+    ref, sabs = oracle.dedisperse(series[None], table, total, want_sabs=True)
+    h_series = torch.from_numpy(series).pin_memory()
+    h_out = torch.full((s.nr_dms, total), float("nan"), dtype=torch.float32).pin_memory()
+    for b in range(nblk):
+        plan.stream_block_async(h_series, series.shape[1], h_out, total, b * S)
+        assert plan.stream_h2d_bytes == s.nr_channels * (S + (M if b == 0 else 0)) * 4
+    plan.host_sync()
+    err = np.abs(h_out.numpy().astype(np.float64) - ref[0])
+    assert (err <= TOL * sabs[0]).all()
     plan.destroy()
 
 
