@@ -40,8 +40,20 @@ LDS_WORDS_PER_SM = 32            # shared memory: 128 bytes per clock and SM
 FALLBACK_HBM_GBS = 6650.0        # B200_PROFILING.md fallback
 FALLBACK_SM_MHZ = 1965.0
 # dram__bytes_read.sum + dram__bytes_write.sum per step, from the ncu --set full captures summarised
-# under profiles/ (the table names the file each number comes from; profiles/r02_traffic.md)
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+# under profiles/ (the table names the file each number comes from; profiles/r03_traffic.md)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic.csv")
+KERNEL_SOURCES = ("kernels.cuh", "kernel_tree.cuh", "gen_tree.py", "variant_defs.cuh", "shift_table.cu")
+
+
+def kernel_sources_sha16():
+    """First 16 hex digits of a SHA-256 over the kernel sources: ties an ncu capture to the code it measured."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_1601_01165_b200", "csrc")
+    for f in KERNEL_SOURCES:
+        h.update(f.encode())
+        h.update(open(os.path.join(base, f), "rb").read())
+    return h.hexdigest()[:16]
 
 
 def measured_peaks():
@@ -65,6 +77,8 @@ def ncu_traffic(config_name, variant_name):
         return None, None
     if d["variant"] != variant_name:
         return None, "profiles capture is of another variant: " + d["variant"]
+    if d.get("kernel_sources_sha16") != kernel_sources_sha16():
+        return None, "profiles capture predates the current kernel sources (sha %s)" % d.get("kernel_sources_sha16")
     return int(d["dram_bytes_per_step"]), d["source"]
 
 

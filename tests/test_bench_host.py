@@ -52,6 +52,8 @@ def test_traffic_table_names_shipped_winners_and_existing_summaries():
     for name, r in rows.items():
         assert r["variant"] in shipped, "the captured variant of %s is not a shipped winner" % name
         assert os.path.exists(os.path.join(ROOT, r["source"].split(" ")[0]))
+        # the capture is of the kernel sources as they are now: editing a kernel without a new ncu capture fails here
+        assert r["kernel_sources_sha16"] == bench.kernel_sources_sha16(), "re-capture profiles/r03_traffic.csv"
         got, src = bench.ncu_traffic(name, r["variant"])
         assert got == int(r["dram_bytes_per_step"]) and src == r["source"]
         assert bench.ncu_traffic(name, "some other variant")[0] is None
